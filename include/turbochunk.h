@@ -1,0 +1,199 @@
+/*
+ * turbochunk.h — C ABI of the B200-native coalesced chunk-processing library.
+ *
+ * The library implements, for ONE GPU, the data-parallel hot path of TurboServe
+ * (arxiv/paper_2606_19271): coalesced chunk processing over persistent per-session
+ * state.  Citations are PAPER.md:<line> (+ section) or SURVEY.md §8 readings (Rn),
+ * which DESIGN.md lists.
+ *
+ *   PAPER.md:66  §3.1  coalesced execution: (i) collect ready sessions, (ii) group them
+ *                      into one coalesced chunk batch, (iii) invoke the model once and write
+ *                      the generated chunks and updated states back per session.
+ *   PAPER.md:74  §3.1  session states execution / suspend / terminate; lifecycle operations
+ *                      initialization, suspension, resumption, termination.
+ *   PAPER.md:76  §3.1  GPU-CPU state offloading: copy state to host, mark suspended and release
+ *                      the GPU slot, restore before generation resumes.
+ *   PAPER.md:261 §6.1  isolated per-session state regions (incl. "temporal or KV-cache states")
+ *                      and a session ownership table.
+ *
+ * Conventions
+ *   - Every call returns TS_OK (0) or a negative ts_status.  No C++ exception crosses the ABI.
+ *   - All-or-nothing: a call validates its whole batch and its page demand before it mutates
+ *     anything; on error no host or device state has changed.
+ *   - Host metadata (page tables, lengths, states, free list) mutates synchronously, in program
+ *     order, at call time.  Device effects are stream-ordered: the library orders its side
+ *     (offload) stream against the caller's compute stream with events, never with host waits
+ *     (ts_offload_sync excepted).
+ *   - Threading: one caller thread per pool.  Compute calls of one pool that are issued on
+ *     different streams must be ordered by the caller.
+ *   - Pointers named *device* are CUDA device pointers on the pool's device; *host* are host
+ *     pointers.  bf16 tensors are raw 16-bit patterns.  The caller owns Q/K/V/O/LSE buffers and
+ *     must keep them alive until the stream reaches the call.
+ *   - No fallback: an unsupported shape is TS_ERR_INVALID, never a slow path.  Without a CUDA
+ *     device every compute call fails with TS_ERR_CUDA.
+ *
+ * Notation: H heads, D head_dim, B page_tokens, T frame_tokens, W window_frames,
+ * NL layers.  Per session: P cached frames, L = P*T cached tokens, o = dead slots at the head of
+ * the first page (0 <= o < B), PT = page table (physical ids, logical order).  Logical token j
+ * lives at page PT[(o+j) div B], slot (o+j) mod B  (R7).
+ */
+#ifndef TURBOCHUNK_H_
+#define TURBOCHUNK_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ts_pool ts_pool; /* opaque */
+
+typedef enum ts_status {
+  TS_OK = 0,
+  TS_ERR_INVALID = -1,  /* null pointer, bad shape/layer, duplicate sid in a batch, chunk_frames < 1 or > W */
+  TS_ERR_STATE = -2,    /* session closed / not RESIDENT for attention, append, suspend / not SUSPENDED for resume */
+  TS_ERR_NO_PAGES = -3, /* device page demand exceeds the free list */
+  TS_ERR_NO_HOST = -4,  /* pinned host arena cannot hold the suspended pages */
+  TS_ERR_CAPACITY = -5, /* no free session id, or batch larger than max_sessions */
+  TS_ERR_CUDA = -6      /* a CUDA runtime/driver call failed (see ts_last_cuda_error) */
+} ts_status;
+
+enum { TS_SESSION_CLOSED = 0, TS_SESSION_RESIDENT = 1, TS_SESSION_SUSPENDED = 2 };
+
+/* ts_kv_append flags */
+enum { TS_COMMIT = 1u }; /* advance P by chunk_frames and roll the window (R14: pass on the last layer of a step) */
+
+typedef struct ts_pool_config {
+  int32_t n_layers;      /* NL >= 1 */
+  int32_t n_heads;       /* H >= 1 */
+  int32_t head_dim;      /* D in {64, 128} */
+  int32_t page_tokens;   /* B: power of two, 16 <= B <= 1024 */
+  int32_t n_pages;       /* physical pages; one page holds B tokens of K and V for all heads and all layers */
+  int32_t frame_tokens;  /* T >= 1 */
+  int32_t window_frames; /* W; <= 0 means no rolling-window cap */
+  int32_t max_sessions;  /* cap on live (resident + suspended) sessions and on the batch size ("bounded") */
+  int32_t device;        /* CUDA device ordinal */
+  int32_t reserved;
+  /* Optional permutation of 0..n_pages-1 = initial FIFO free-list order (R8, R9). NULL = identity. Copied. */
+  const int32_t* free_order; /* host */
+  /* KV slab: device memory of at least ts_pool_slab_bytes() bytes, 1024-byte aligned.  NULL: the library
+   * allocates it with cudaMalloc.  Caller-provided memory (e.g. a torch tensor) stays owned by the caller
+   * and must outlive the pool. */
+  void* kv_slab;          /* device */
+  int64_t kv_slab_bytes;
+  /* Pinned host arena for suspended sessions, in whole pages of ts_pool_page_bytes().  NULL with
+   * host_bytes > 0: the library allocates it with cudaHostAlloc. */
+  void* host_arena;       /* host, page-locked */
+  int64_t host_bytes;
+  /* Side stream (cudaStream_t) for suspend/resume copies.  NULL: the library creates a non-blocking one. */
+  void* side_stream;
+} ts_pool_config;
+
+typedef struct ts_session_info_t {
+  int32_t state;       /* TS_SESSION_* */
+  int32_t frames;      /* P */
+  int64_t len_tokens;  /* L = P*T */
+  int32_t head_off;    /* o */
+  int32_t n_pages;     /* |PT| (saved page count while suspended) */
+} ts_session_info_t;
+
+typedef struct ts_pool_stats_t {
+  int32_t free_pages;
+  int32_t resident;
+  int32_t suspended;
+  int32_t host_pages_used;
+  int32_t host_pages_cap;
+  int32_t reserved;
+  int64_t page_bytes;
+} ts_pool_stats_t;
+
+/* Layout helpers (pure host arithmetic; usable without a GPU). Return < 0 on an invalid config. */
+int64_t ts_pool_page_bytes(const ts_pool_config* cfg); /* NL * 2 * H * B * D * 2 */
+int64_t ts_pool_slab_bytes(const ts_pool_config* cfg); /* n_pages * page bytes */
+
+/* create the per-GPU pool: KV slab, free list, session table, offload arena, side stream. */
+int ts_pool_create(const ts_pool_config* cfg, ts_pool** out);
+int ts_pool_destroy(ts_pool* pool);
+
+/* PAPER.md:74 "initialization": new session with the lowest free id (R13), P = o = 0, empty PT, RESIDENT. */
+int ts_session_open(ts_pool* pool, int32_t* sid_out);
+/* PAPER.md:74 "termination": releases every resource.  Legal from RESIDENT (pages pushed to the back of
+ * the free list in logical order) or SUSPENDED (host copy dropped). */
+int ts_session_close(ts_pool* pool, int32_t sid);
+
+/*
+ * PAPER.md:66 (i)-(iii), the attention contraction inside "invokes the model once for the batch".
+ * For each session sids[b] (all RESIDENT, no duplicates), head h and chunk token i (frame f = i div T):
+ *   out[i,h,:] = softmax_j( scale * <q[i,h,:], k_j> ) . v_j   over the visible keys j =
+ *     the session's cached tokens of its last min(P, W - c) frames (whole cache if W <= 0)  (R6)
+ *     U the chunk's own tokens of frames <= f  (frame-block-causal, R1).
+ * bf16 operands, fp32 accumulation and fp32 online softmax, bf16 output (R3, R4).
+ *   q, k, v, out : device bf16 [sum_b C_b][H][D], sessions concatenated in sids order, no padding (R15);
+ *                  C_b = chunk_frames[b] * T.  16-byte aligned.
+ *   lse          : device fp32 [sum_b C_b][H] natural-log logsumexp of the scaled logits, or NULL.
+ *   scale        : softmax scale (R2).
+ *   cuda_stream  : cudaStream_t of the caller (NULL = legacy default stream).
+ * Does not change pool state (R5).  Waits (stream-side) for a pending resume of any session in the batch.
+ * n == 0 is a no-op.
+ */
+int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*host*/,
+                       const int32_t* chunk_frames /*host*/, const void* q, const void* k, const void* v,
+                       void* out, float* lse, float scale, void* cuda_stream);
+
+/*
+ * PAPER.md:66 (iii) "writes the generated chunks and updated states back to their corresponding sessions".
+ * Sessions in sids order: grow PT by ceil((o+L+C)/B) - |PT| pages popped from the front of the free list
+ * (idempotent across the layers of one step), scatter the chunk's K/V to logical positions [L, L+C) of
+ * `layer` (byte-exact 128-bit copies).  With TS_COMMIT: P += c, then roll the window: evict e = max(0, P - W)
+ * oldest whole frames, o += e*T, pages whose slots are all dead go to the back of the free list (R6, R10).
+ *   k, v : device bf16 [sum_b C_b][H][D] as above.
+ */
+int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*host*/,
+                 const int32_t* chunk_frames /*host*/, const void* k, const void* v, uint32_t flags,
+                 void* cuda_stream);
+
+/*
+ * One coalesced chunk step with HOST buffers (the end-to-end entry point): copies q,k,v from (pinned) host
+ * memory to device staging owned by the pool, runs ts_chunk_attention and ts_kv_append(flags) on
+ * `cuda_stream`, copies `out` back to out_host.  All copies are enqueued on `cuda_stream`; the call returns
+ * without waiting.  Staging grows on demand (cudaMalloc) and is reused.
+ */
+int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
+                       const void* q_host, const void* k_host, const void* v_host, void* out_host,
+                       float scale, uint32_t flags, void* cuda_stream);
+
+/* PAPER.md:76 (i)-(ii): copy the session's pages (every layer, whole pages, logical order — R11) to the pinned
+ * arena on the side stream, after the compute-stream work already enqueued on that session; mark SUSPENDED;
+ * push its page ids to the back of the free list in logical order.  A freed page is not handed to a later
+ * writer before the copy out of it has completed (event-ordered). */
+int ts_session_suspend(ts_pool* pool, int32_t sid);
+/* PAPER.md:76 (iii): pop the saved number of pages from the front of the free list, copy the host pages back
+ * on the side stream, mark RESIDENT.  Later compute calls on the session wait (stream-side) for the copy. */
+int ts_session_resume(ts_pool* pool, int32_t sid);
+/* Host-blocks until all side-stream work enqueued so far has completed. */
+int ts_offload_sync(ts_pool* pool);
+
+/* Introspection (parity is taken on these, never on raw slabs: the physical layout is private). */
+int ts_session_info(ts_pool* pool, int32_t sid, ts_session_info_t* out);
+/* Copies up to `cap` page ids (logical order) to `out` (host); *n_out = |PT|. */
+int ts_session_page_table(ts_pool* pool, int32_t sid, int32_t* out, int32_t cap, int32_t* n_out);
+/* Logical K and V of a RESIDENT session, device bf16 [L][H][D] each, gathered through the page table. */
+int ts_gather_kv(ts_pool* pool, int32_t layer, int32_t sid, void* k_out, void* v_out, void* cuda_stream);
+/* Copies up to `cap` ids of the free list, front first. */
+int ts_pool_free_list(ts_pool* pool, int32_t* out, int32_t cap, int32_t* n_out);
+int ts_pool_stats(ts_pool* pool, ts_pool_stats_t* out);
+/* The side stream in use (cudaStream_t), for timing offload with events. */
+void* ts_pool_side_stream(ts_pool* pool);
+/* Number of kernels the library has launched on this pool since creation (bench.py's gpu_launches). */
+int64_t ts_pool_launch_count(ts_pool* pool);
+
+const char* ts_strerror(int code);
+/* Text of the last CUDA error seen by this pool's calls on this thread ("" if none). */
+const char* ts_last_cuda_error(void);
+/* Library version string. */
+const char* ts_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TURBOCHUNK_H_ */

@@ -1,0 +1,236 @@
+"""ctypes binding of include/turbochunk.h.  Same names as the C ABI; marshalling only.
+
+Tensors are torch tensors (bf16 or any 16-bit dtype for K/V/Q/O, fp32 for LSE); device memory for the KV
+slab and pinned memory for the offload arena are allocated with torch and handed to the library as raw
+pointers.  No step of the path is computed in Python.
+"""
+import ctypes as C
+import os
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+lib_path = os.path.join(HERE, "libturbochunk.so")
+
+TS_OK, TS_ERR_INVALID, TS_ERR_STATE, TS_ERR_NO_PAGES, TS_ERR_NO_HOST, TS_ERR_CAPACITY, TS_ERR_CUDA = 0, -1, -2, -3, -4, -5, -6
+TS_SESSION_CLOSED, TS_SESSION_RESIDENT, TS_SESSION_SUSPENDED = 0, 1, 2
+TS_COMMIT = 1
+
+EXPORTED_SYMBOLS = [
+    "ts_pool_page_bytes", "ts_pool_slab_bytes", "ts_pool_create", "ts_pool_destroy", "ts_session_open",
+    "ts_session_close", "ts_chunk_attention", "ts_kv_append", "ts_chunk_step_host", "ts_session_suspend",
+    "ts_session_resume", "ts_offload_sync", "ts_session_info", "ts_session_page_table", "ts_gather_kv",
+    "ts_pool_free_list", "ts_pool_stats", "ts_pool_side_stream", "ts_pool_launch_count", "ts_strerror",
+    "ts_last_cuda_error", "ts_version",
+]
+
+
+class ts_pool_config(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("n_heads", C.c_int32), ("head_dim", C.c_int32), ("page_tokens", C.c_int32),
+                ("n_pages", C.c_int32), ("frame_tokens", C.c_int32), ("window_frames", C.c_int32),
+                ("max_sessions", C.c_int32), ("device", C.c_int32), ("reserved", C.c_int32),
+                ("free_order", C.POINTER(C.c_int32)), ("kv_slab", C.c_void_p), ("kv_slab_bytes", C.c_int64),
+                ("host_arena", C.c_void_p), ("host_bytes", C.c_int64), ("side_stream", C.c_void_p)]
+
+
+class ts_session_info_t(C.Structure):
+    _fields_ = [("state", C.c_int32), ("frames", C.c_int32), ("len_tokens", C.c_int64), ("head_off", C.c_int32),
+                ("n_pages", C.c_int32)]
+
+
+class ts_pool_stats_t(C.Structure):
+    _fields_ = [("free_pages", C.c_int32), ("resident", C.c_int32), ("suspended", C.c_int32),
+                ("host_pages_used", C.c_int32), ("host_pages_cap", C.c_int32), ("reserved", C.c_int32),
+                ("page_bytes", C.c_int64)]
+
+
+def _load():
+    if not os.path.exists(lib_path):
+        raise ImportError(f"{lib_path} is missing: run `python -m paper_2606_19271_b200.build` "
+                          "(or __graft_entry__.build()). There is no fallback path.")
+    L = C.CDLL(lib_path)
+    P = C.c_void_p
+    I32P = C.POINTER(C.c_int32)
+    L.ts_pool_page_bytes.restype = C.c_int64
+    L.ts_pool_page_bytes.argtypes = [C.POINTER(ts_pool_config)]
+    L.ts_pool_slab_bytes.restype = C.c_int64
+    L.ts_pool_slab_bytes.argtypes = [C.POINTER(ts_pool_config)]
+    L.ts_pool_create.argtypes = [C.POINTER(ts_pool_config), C.POINTER(P)]
+    L.ts_pool_destroy.argtypes = [P]
+    L.ts_session_open.argtypes = [P, I32P]
+    L.ts_session_close.argtypes = [P, C.c_int32]
+    L.ts_chunk_attention.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, P, P, P, C.c_float, P]
+    L.ts_kv_append.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, C.c_uint32, P]
+    L.ts_chunk_step_host.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, P, P, C.c_float, C.c_uint32, P]
+    L.ts_session_suspend.argtypes = [P, C.c_int32]
+    L.ts_session_resume.argtypes = [P, C.c_int32]
+    L.ts_offload_sync.argtypes = [P]
+    L.ts_session_info.argtypes = [P, C.c_int32, C.POINTER(ts_session_info_t)]
+    L.ts_session_page_table.argtypes = [P, C.c_int32, I32P, C.c_int32, I32P]
+    L.ts_gather_kv.argtypes = [P, C.c_int32, C.c_int32, P, P, P]
+    L.ts_pool_free_list.argtypes = [P, I32P, C.c_int32, I32P]
+    L.ts_pool_stats.argtypes = [P, C.POINTER(ts_pool_stats_t)]
+    L.ts_pool_side_stream.restype = P
+    L.ts_pool_side_stream.argtypes = [P]
+    L.ts_pool_launch_count.restype = C.c_int64
+    L.ts_pool_launch_count.argtypes = [P]
+    L.ts_strerror.restype = C.c_char_p
+    L.ts_strerror.argtypes = [C.c_int]
+    L.ts_last_cuda_error.restype = C.c_char_p
+    L.ts_version.restype = C.c_char_p
+    return L
+
+
+lib = _load()
+
+
+class TurboChunkError(RuntimeError):
+    def __init__(self, code, where):
+        detail = lib.ts_last_cuda_error().decode() if code == TS_ERR_CUDA else ""
+        super().__init__(f"{where}: {lib.ts_strerror(code).decode()} ({code}) {detail}".strip())
+        self.code = code
+
+
+def _check(code, where):
+    if code != TS_OK:
+        raise TurboChunkError(code, where)
+
+
+def _i32(values):
+    arr = (C.c_int32 * max(1, len(values)))(*[int(x) for x in values])
+    return arr
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+class TurboChunkPool:
+    """Owns a ts_pool and the torch memory behind it.  Methods mirror the C ABI one to one."""
+
+    def __init__(self, n_layers, n_heads, head_dim, page_tokens, n_pages, frame_tokens, window_frames,
+                 max_sessions, free_order=None, host_pages=0, device=0):
+        cfg = ts_pool_config()
+        cfg.n_layers, cfg.n_heads, cfg.head_dim, cfg.page_tokens = n_layers, n_heads, head_dim, page_tokens
+        cfg.n_pages, cfg.frame_tokens, cfg.window_frames, cfg.max_sessions = n_pages, frame_tokens, window_frames, max_sessions
+        cfg.device = device
+        page_bytes = lib.ts_pool_page_bytes(C.byref(cfg))
+        if page_bytes < 0:
+            raise TurboChunkError(int(page_bytes), "ts_pool_page_bytes")
+        self.page_bytes = int(page_bytes)
+        slab_bytes = int(lib.ts_pool_slab_bytes(C.byref(cfg)))
+        self.device = torch.device("cuda", device)
+        # device memory and pinned memory come from torch (PyTorch is the allocator, not the product)
+        self._slab = torch.empty(slab_bytes + 1024, dtype=torch.uint8, device=self.device)
+        base = self._slab.data_ptr()
+        aligned = (base + 1023) // 1024 * 1024
+        cfg.kv_slab = aligned
+        cfg.kv_slab_bytes = slab_bytes
+        self._host = None
+        if host_pages > 0:
+            self._host = torch.empty(host_pages * self.page_bytes, dtype=torch.uint8, pin_memory=True)
+            cfg.host_arena = self._host.data_ptr()
+            cfg.host_bytes = host_pages * self.page_bytes
+        self._free_order = None
+        if free_order is not None:
+            self._free_order = _i32(list(free_order))
+            cfg.free_order = C.cast(self._free_order, C.POINTER(C.c_int32))
+        self._side = torch.cuda.Stream(device=self.device)
+        cfg.side_stream = self._side.cuda_stream
+        self.cfg = cfg
+        self.shape = (n_layers, n_heads, head_dim, page_tokens, n_pages, frame_tokens, window_frames, max_sessions)
+        handle = C.c_void_p()
+        _check(lib.ts_pool_create(C.byref(cfg), C.byref(handle)), "ts_pool_create")
+        self._h = handle
+
+    # ---- lifecycle
+    def close(self):
+        if getattr(self, "_h", None):
+            lib.ts_pool_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def ts_session_open(self):
+        sid = C.c_int32(-1)
+        _check(lib.ts_session_open(self._h, C.byref(sid)), "ts_session_open")
+        return sid.value
+
+    def ts_session_close(self, sid):
+        _check(lib.ts_session_close(self._h, sid), "ts_session_close")
+
+    # ---- hot path
+    def ts_chunk_attention(self, layer, sids, chunk_frames, q, k, v, out, lse=None, scale=1.0, stream=None):
+        _check(lib.ts_chunk_attention(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(q), _ptr(k),
+                                      _ptr(v), _ptr(out), _ptr(lse), C.c_float(float(scale)), _stream(stream)),
+               "ts_chunk_attention")
+
+    def ts_kv_append(self, layer, sids, chunk_frames, k, v, flags=TS_COMMIT, stream=None):
+        _check(lib.ts_kv_append(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(k), _ptr(v),
+                                C.c_uint32(flags), _stream(stream)), "ts_kv_append")
+
+    def ts_chunk_step_host(self, layer, sids, chunk_frames, q_host, k_host, v_host, out_host, scale, flags=TS_COMMIT,
+                           stream=None):
+        _check(lib.ts_chunk_step_host(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(q_host),
+                                      _ptr(k_host), _ptr(v_host), _ptr(out_host), C.c_float(float(scale)),
+                                      C.c_uint32(flags), _stream(stream)), "ts_chunk_step_host")
+
+    def ts_session_suspend(self, sid):
+        _check(lib.ts_session_suspend(self._h, sid), "ts_session_suspend")
+
+    def ts_session_resume(self, sid):
+        _check(lib.ts_session_resume(self._h, sid), "ts_session_resume")
+
+    def ts_offload_sync(self):
+        _check(lib.ts_offload_sync(self._h), "ts_offload_sync")
+
+    # ---- introspection
+    def ts_session_info(self, sid):
+        info = ts_session_info_t()
+        _check(lib.ts_session_info(self._h, sid, C.byref(info)), "ts_session_info")
+        return {"state": info.state, "frames": info.frames, "len_tokens": info.len_tokens,
+                "head_off": info.head_off, "n_pages": info.n_pages}
+
+    def ts_session_page_table(self, sid):
+        n = C.c_int32(0)
+        _check(lib.ts_session_page_table(self._h, sid, None, 0, C.byref(n)), "ts_session_page_table")
+        buf = (C.c_int32 * max(1, n.value))()
+        _check(lib.ts_session_page_table(self._h, sid, buf, n.value, C.byref(n)), "ts_session_page_table")
+        return [buf[i] for i in range(n.value)]
+
+    def ts_pool_free_list(self):
+        n = C.c_int32(0)
+        _check(lib.ts_pool_free_list(self._h, None, 0, C.byref(n)), "ts_pool_free_list")
+        buf = (C.c_int32 * max(1, n.value))()
+        _check(lib.ts_pool_free_list(self._h, buf, n.value, C.byref(n)), "ts_pool_free_list")
+        return [buf[i] for i in range(n.value)]
+
+    def ts_gather_kv(self, layer, sid, stream=None):
+        info = self.ts_session_info(sid)
+        H, D = self.shape[1], self.shape[2]
+        k = torch.empty((info["len_tokens"], H, D), dtype=torch.bfloat16, device=self.device)
+        v = torch.empty_like(k)
+        _check(lib.ts_gather_kv(self._h, layer, sid, _ptr(k), _ptr(v), _stream(stream)), "ts_gather_kv")
+        return k, v
+
+    def ts_pool_stats(self):
+        st = ts_pool_stats_t()
+        _check(lib.ts_pool_stats(self._h, C.byref(st)), "ts_pool_stats")
+        return {f: getattr(st, f) for f, _ in ts_pool_stats_t._fields_ if f != "reserved"}
+
+    def ts_pool_launch_count(self):
+        return int(lib.ts_pool_launch_count(self._h))
+
+    @property
+    def side_stream(self):
+        return self._side

@@ -1,0 +1,406 @@
+// Coalesced chunk attention for sm_100a (step a2 of SURVEY.md §8(a); PAPER.md:66 (iii)).
+//
+// One persistent CTA per SM walks a host-balanced list of work items (session, head, pair of 128-row
+// query tiles).  Per item the KV sequence is: the session's visible cached tokens in PHYSICAL page order
+// (softmax is order-invariant over keys), gathered page by page through the page table with TMA, then the
+// chunk's own K/V tiles from the packed call tensors.  Only the first/last cache tile and the chunk tiles
+// that cross a frame boundary take the masked path.
+//
+// Warp roles (384 threads):
+//   warp 0      TMA producer   Q tiles once per item, K/V tiles into a ring of kSlots smem slots
+//   warp 1      MMA issuer     tcgen05.mma, one elected thread; S = Q K^T (SS), O += P V (TS, P in TMEM)
+//   warps 4-7   softmax for query tile 0 (one thread per row): online softmax in fp32, lazy rescale of O,
+//   warps 8-11  softmax for query tile 1                        P written back to TMEM as bf16, epilogue
+// TMEM (512 columns): S0 [0,128) / P0 aliases [0,64); S1 [128,256) / P1; O0 [256,256+D); O1 [256+D,256+2D).
+// Issue order  S0(0) S1(0) | PV0(j) S0(j+1) PV1(j) S1(j+1) | ...  keeps the tensor pipe busy while the
+// other tile's softmax runs (two-tile ping-pong).
+#include "internal.h"
+#include "ptx.cuh"
+
+namespace tc {
+
+constexpr int kThreads = 384;
+constexpr int kTmemCols = 512;
+constexpr float kRescaleThresholdLog2 = 8.0f;   // lazy rescale: tolerate p up to 2^8 before touching O
+
+template <int D>
+struct Cfg {
+  static constexpr int kTileBytes = 128 * D * 2;        // one [128 x D] bf16 tile
+  static constexpr int kDBlocks = D / 64;               // 64-column (128-byte) swizzle blocks per tile
+  static constexpr int kBlockBytes = 128 * 128;         // one [128 rows x 128 B] swizzle block
+  static constexpr int kSlots = (D == 128) ? 5 : 8;
+  static constexpr int kSmemQ = 2 * kTileBytes;
+  static constexpr int kSmemKV = kSlots * kTileBytes;
+  static constexpr int kNumBars = 2 * kSlots + 2 + 8;
+  static constexpr int kSmemBytes = 1024 + kSmemQ + kSmemKV + kNumBars * 8 + 16;
+};
+
+struct ItemGeom {
+  int sess, head, r0, n_q, C, q_off, pt_off, n_pt;
+  int x_begin, x_end, t0, n_prior, n_chunk, n_kv;
+};
+
+__device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int idx) {
+  const WorkItem w = p.items[idx];
+  const SessDesc s = p.sess[w.sess];
+  ItemGeom g;
+  g.sess = w.sess;
+  g.head = w.head;
+  g.r0 = w.q_pair * 256;
+  g.C = s.C;
+  g.q_off = s.q_off;
+  g.pt_off = s.pt_off;
+  g.n_pt = s.n_pt;
+  g.x_begin = s.x_begin;
+  g.x_end = s.x_end;
+  g.n_q = (g.r0 + 128 < s.C) ? 2 : 1;
+  const int last_row = min(s.C, g.r0 + 256) - 1;
+  const int kv_hi = min(s.C, (last_row / p.T + 1) * p.T);   // chunk keys visible to the item's last row
+  g.n_chunk = (kv_hi + 127) >> 7;
+  if (s.x_end > s.x_begin) {
+    g.t0 = s.x_begin >> 7;
+    g.n_prior = ((s.x_end - 1) >> 7) - g.t0 + 1;
+  } else {
+    g.t0 = 0;
+    g.n_prior = 0;
+  }
+  g.n_kv = g.n_prior + g.n_chunk;
+  return g;
+}
+
+template <int D>
+__global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __grid_constant__ AttnParams p) {
+  using C = Cfg<D>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* sQ = smem;
+  uint8_t* sKV = smem + C::kSmemQ;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + C::kSmemKV);
+  uint64_t* kv_full = bars;
+  uint64_t* kv_empty = bars + C::kSlots;
+  uint64_t* q_full = bars + 2 * C::kSlots;
+  uint64_t* q_empty = q_full + 1;
+  uint64_t* s_full = q_full + 2;    // [2]
+  uint64_t* p_full = q_full + 4;    // [2]
+  uint64_t* o_done = q_full + 6;    // [2]
+  uint64_t* o_free = q_full + 8;    // [2]
+  uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + C::kNumBars);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    for (int i = 0; i < C::kSlots; ++i) {
+      mbar_init(&kv_full[i], 1);
+      mbar_init(&kv_empty[i], 1);
+    }
+    mbar_init(q_full, 1);
+    mbar_init(q_empty, 1);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(&s_full[i], 1);
+      mbar_init(&p_full[i], 128);
+      mbar_init(&o_done[i], 1);
+      mbar_init(&o_free[i], 128);
+    }
+    fence_mbar_init();
+    tma_prefetch_desc(&p.map_k);
+    tma_prefetch_desc(&p.map_v);
+  }
+  if (warp == 1) tmem_alloc(tmem_ptr, kTmemCols);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_ptr;
+
+  const int it_begin = p.cta_begin[blockIdx.x];
+  const int it_end = p.cta_begin[blockIdx.x + 1];
+
+  if (warp == 0) {
+    // ===================================================================== TMA producer
+    if (lane == 0) {
+      uint32_t kv_it = 0;
+      uint32_t item_cnt = 0;
+      for (int idx = it_begin; idx < it_end; ++idx, ++item_cnt) {
+        const ItemGeom g = decode_item(p, idx);
+        const CUtensorMap* mq = p.sess_maps + g.sess * 3;
+        const CUtensorMap* mkn = mq + 1;
+        const CUtensorMap* mvn = mq + 2;
+        const int32_t* pt = p.page_tables + g.pt_off;
+        mbar_wait(q_empty, (item_cnt & 1) ^ 1);
+        mbar_arrive_expect_tx(q_full, g.n_q * C::kTileBytes);
+        for (int i = 0; i < g.n_q; ++i)
+          for (int b = 0; b < C::kDBlocks; ++b)
+            tma_load_3d(sQ + i * C::kTileBytes + b * C::kBlockBytes, mq, 64 * b, g.head, g.r0 + 128 * i, q_full);
+        for (int j = 0; j < g.n_kv; ++j) {
+          for (int kv = 0; kv < 2; ++kv, ++kv_it) {
+            const uint32_t slot = kv_it % C::kSlots;
+            const uint32_t ph = (kv_it / C::kSlots) & 1;
+            mbar_wait(&kv_empty[slot], ph ^ 1);
+            mbar_arrive_expect_tx(&kv_full[slot], C::kTileBytes);
+            uint8_t* dst = sKV + slot * C::kTileBytes;
+            if (j < g.n_prior) {
+              const CUtensorMap* mc = kv ? &p.map_v : &p.map_k;
+              const int t = g.t0 + j;
+              if (p.B >= 128) {
+                const int x = t << 7;
+                const int page = pt[x >> p.log2_B];
+                const int tok0 = x & (p.B - 1);
+                for (int b = 0; b < C::kDBlocks; ++b)
+                  tma_load_4d(dst + b * C::kBlockBytes, mc, 64 * b, tok0, g.head, page, &kv_full[slot]);
+              } else {
+                const int per = 128 >> p.log2_B;      // pages per 128-key tile
+                for (int s = 0; s < per; ++s) {
+                  const int pidx = min(t * per + s, g.n_pt - 1);   // past-the-end sub-tiles re-read the last page (masked)
+                  const int page = pt[pidx];
+                  for (int b = 0; b < C::kDBlocks; ++b)
+                    tma_load_4d(dst + b * C::kBlockBytes + s * p.B * 128, mc, 64 * b, 0, g.head, page, &kv_full[slot]);
+                }
+              }
+            } else {
+              const int u = j - g.n_prior;
+              const CUtensorMap* mc = kv ? mvn : mkn;
+              for (int b = 0; b < C::kDBlocks; ++b)
+                tma_load_3d(dst + b * C::kBlockBytes, mc, 64 * b, g.head, 128 * u, &kv_full[slot]);
+            }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================================================================== MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc_s = make_idesc_bf16(128, 128, 0, 0);
+      constexpr uint32_t idesc_pv = make_idesc_bf16(128, D, 0, 1);
+      const uint32_t sQ_addr = smem_u32(sQ);
+      const uint32_t sKV_addr = smem_u32(sKV);
+      auto issue_s = [&](int i, uint32_t slot) {
+        const uint32_t a = sQ_addr + i * C::kTileBytes;
+        const uint32_t b = sKV_addr + slot * C::kTileBytes;
+#pragma unroll
+        for (int kk = 0; kk < D / 16; ++kk) {
+          const uint32_t off = (kk >> 2) * C::kBlockBytes + (kk & 3) * 32;
+          mma_ss(tmem_base + i * 128, make_smem_desc_sw128(a + off, 16, 1024), make_smem_desc_sw128(b + off, 16, 1024),
+                 idesc_s, kk > 0);
+        }
+      };
+      auto issue_pv = [&](int i, uint32_t slot, bool acc) {
+        const uint32_t b = sKV_addr + slot * C::kTileBytes;
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk)
+          mma_ts(tmem_base + 256 + i * D, tmem_base + i * 128 + kk * 8,
+                 make_smem_desc_sw128(b + kk * 2048, C::kBlockBytes, 1024), idesc_pv, (acc || kk > 0) ? 1u : 0u);
+      };
+      uint32_t kv_it = 0, item_cnt = 0;
+      uint32_t cnt_p[2] = {0, 0};
+      uint32_t cnt_items[2] = {0, 0};
+      for (int idx = it_begin; idx < it_end; ++idx, ++item_cnt) {
+        const ItemGeom g = decode_item(p, idx);
+        mbar_wait(q_full, item_cnt & 1);
+        {
+          const uint32_t slot = kv_it % C::kSlots, ph = (kv_it / C::kSlots) & 1;
+          ++kv_it;
+          mbar_wait(&kv_full[slot], ph);
+          tc_fence_after();
+          for (int i = 0; i < g.n_q; ++i) {
+            issue_s(i, slot);
+            mma_commit(&s_full[i]);
+          }
+          mma_commit(&kv_empty[slot]);
+          if (g.n_kv == 1) mma_commit(q_empty);
+        }
+        for (int j = 0; j < g.n_kv; ++j) {
+          const uint32_t slot_v = kv_it % C::kSlots, ph_v = (kv_it / C::kSlots) & 1;
+          ++kv_it;
+          const bool has_next = (j + 1 < g.n_kv);
+          uint32_t slot_k = 0, ph_k = 0;
+          if (has_next) {
+            slot_k = kv_it % C::kSlots;
+            ph_k = (kv_it / C::kSlots) & 1;
+            ++kv_it;
+          }
+          for (int i = 0; i < g.n_q; ++i) {
+            mbar_wait(&p_full[i], cnt_p[i] & 1);
+            ++cnt_p[i];
+            if (i == 0) mbar_wait(&kv_full[slot_v], ph_v);
+            if (j == 0) mbar_wait(&o_free[i], (cnt_items[i] & 1) ^ 1);
+            tc_fence_after();
+            issue_pv(i, slot_v, j > 0);
+            mma_commit(&o_done[i]);
+            if (i == g.n_q - 1) mma_commit(&kv_empty[slot_v]);
+            if (has_next) {
+              if (i == 0) {
+                mbar_wait(&kv_full[slot_k], ph_k);
+                tc_fence_after();
+              }
+              issue_s(i, slot_k);
+              mma_commit(&s_full[i]);
+              if (i == g.n_q - 1) {
+                mma_commit(&kv_empty[slot_k]);
+                if (j + 2 == g.n_kv) mma_commit(q_empty);
+              }
+            }
+          }
+        }
+        for (int i = 0; i < g.n_q; ++i) ++cnt_items[i];
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================================================================== softmax + epilogue, one thread per query row
+    const int wg = (warp - 4) >> 2;                       // query tile handled by this warpgroup
+    const int row_in_tile = (warp & 3) * 32 + lane;
+    const uint32_t lane_sel = (uint32_t)((warp & 3) * 32) << 16;
+    const uint32_t taddr_s = tmem_base + lane_sel + wg * 128;
+    const uint32_t taddr_o = tmem_base + lane_sel + 256 + wg * D;
+    const float c = p.scale_log2;
+    const float thr = kRescaleThresholdLog2 / c;
+    uint32_t cnt_s = 0, cnt_pv = 0;
+    for (int idx = it_begin; idx < it_end; ++idx) {
+      const ItemGeom g = decode_item(p, idx);
+      if (wg >= g.n_q) continue;
+      const int first_row = g.r0 + 128 * wg;
+      const int row = first_row + row_in_tile;
+      const int lim_row = min(g.C, (min(row, g.C - 1) / p.T + 1) * p.T);   // chunk keys visible to this row
+      const int lim_min = min(g.C, (first_row / p.T + 1) * p.T);           // ... to the tile's first row
+      float m = -INFINITY, l = 0.f;
+      for (int j = 0; j < g.n_kv; ++j) {
+        mbar_wait(&s_full[wg], cnt_s & 1);
+        ++cnt_s;
+        tc_fence_after();
+        uint32_t s[128];
+        tmem_ld32(taddr_s + 0, s + 0);
+        tmem_ld32(taddr_s + 32, s + 32);
+        tmem_ld32(taddr_s + 64, s + 64);
+        tmem_ld32(taddr_s + 96, s + 96);
+        tmem_ld_wait();
+        // ---- mask (rare path)
+        int lo = 0, hi = 128;
+        bool need_mask;
+        if (j < g.n_prior) {
+          if (j == 0) lo = g.x_begin - (g.t0 << 7);
+          if (j == g.n_prior - 1) hi = g.x_end - ((g.t0 + j) << 7);
+          need_mask = (lo > 0) || (hi < 128);
+        } else {
+          const int base = (j - g.n_prior) << 7;
+          need_mask = base + 128 > lim_min;
+          hi = max(0, min(128, lim_row - base));
+        }
+        if (need_mask) {
+#pragma unroll
+          for (int k = 0; k < 128; ++k)
+            if (k < lo || k >= hi) s[k] = 0xff800000u;   // -inf
+        }
+        // ---- row max
+        float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]), mx3 = __uint_as_float(s[3]);
+#pragma unroll
+        for (int k = 4; k < 128; k += 4) {
+          mx0 = fmaxf(mx0, __uint_as_float(s[k]));
+          mx1 = fmaxf(mx1, __uint_as_float(s[k + 1]));
+          mx2 = fmaxf(mx2, __uint_as_float(s[k + 2]));
+          mx3 = fmaxf(mx3, __uint_as_float(s[k + 3]));
+        }
+        const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+        if (j == 0) {
+          m = mx;   // the first tile of an item always holds a visible key for every row
+        } else {
+          const bool need = mx > m + thr;
+          if (__any_sync(0xffffffffu, need)) {
+            // rescale this warp's rows of O in TMEM: needs PV(j-1) of this tile complete
+            const float m_new = fmaxf(m, mx);
+            const float f = ex2_approx((m - m_new) * c);
+            l *= f;
+            m = m_new;
+            mbar_wait(&o_done[wg], (cnt_pv - 1) & 1);
+            tc_fence_after();
+#pragma unroll
+            for (int cc = 0; cc < D; cc += 32) {
+              uint32_t o[32];
+              tmem_ld32(taddr_o + cc, o);
+              tmem_ld_wait();
+#pragma unroll
+              for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * f);
+              tmem_st32(taddr_o + cc, o);
+            }
+          }
+        }
+        // ---- p = exp2(s*c - m*c); row sum; bf16 P back into TMEM (aliases the first 64 columns of S)
+        const float neg_mc = -m * c;
+        float l0 = 0.f, l1 = 0.f;
+#pragma unroll
+        for (int cc = 0; cc < 128; cc += 32) {
+          uint32_t pk[16];
+#pragma unroll
+          for (int k = 0; k < 32; k += 2) {
+            const float p0 = ex2_approx(fmaf(__uint_as_float(s[cc + k]), c, neg_mc));
+            const float p1 = ex2_approx(fmaf(__uint_as_float(s[cc + k + 1]), c, neg_mc));
+            l0 += p0;
+            l1 += p1;
+            pk[k >> 1] = pack_bf16x2(p0, p1);
+          }
+          tmem_st16(taddr_s + (cc >> 1), pk);
+        }
+        l += l0 + l1;
+        tmem_st_wait();
+        tc_fence_before();
+        mbar_arrive(&p_full[wg]);
+        ++cnt_pv;
+      }
+      // ---- epilogue: O / l -> bf16 -> global
+      mbar_wait(&o_done[wg], (cnt_pv - 1) & 1);
+      tc_fence_after();
+      const float inv_l = 1.0f / l;
+      const bool store = row < g.C;
+      uint16_t* orow = p.out + ((size_t)(g.q_off + row) * p.H + g.head) * D;
+#pragma unroll
+      for (int cc = 0; cc < D; cc += 32) {
+        uint32_t o[32];
+        tmem_ld32(taddr_o + cc, o);
+        tmem_ld_wait();
+        if (store) {
+#pragma unroll
+          for (int k = 0; k < 32; k += 8) {
+            uint4 v;
+            v.x = pack_bf16x2(__uint_as_float(o[k + 0]) * inv_l, __uint_as_float(o[k + 1]) * inv_l);
+            v.y = pack_bf16x2(__uint_as_float(o[k + 2]) * inv_l, __uint_as_float(o[k + 3]) * inv_l);
+            v.z = pack_bf16x2(__uint_as_float(o[k + 4]) * inv_l, __uint_as_float(o[k + 5]) * inv_l);
+            v.w = pack_bf16x2(__uint_as_float(o[k + 6]) * inv_l, __uint_as_float(o[k + 7]) * inv_l);
+            *reinterpret_cast<uint4*>(orow + cc + k) = v;
+          }
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(&o_free[wg]);
+      if (p.lse != nullptr && store)
+        p.lse[(size_t)(g.q_off + row) * p.H + g.head] = (m * c + log2f(l)) * 0.6931471805599453f;
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem_base, kTmemCols);
+}
+
+int attention_smem_bytes(int head_dim) { return head_dim == 128 ? Cfg<128>::kSmemBytes : Cfg<64>::kSmemBytes; }
+
+cudaError_t launch_attention(const AttnParams& p, int head_dim, int grid, cudaStream_t stream) {
+  static bool configured[2] = {false, false};
+  if (head_dim == 128) {
+    if (!configured[0]) {
+      cudaError_t e = cudaFuncSetAttribute(chunk_attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           Cfg<128>::kSmemBytes);
+      if (e != cudaSuccess) return e;
+      configured[0] = true;
+    }
+    chunk_attention_kernel<128><<<grid, kThreads, Cfg<128>::kSmemBytes, stream>>>(p);
+  } else {
+    if (!configured[1]) {
+      cudaError_t e = cudaFuncSetAttribute(chunk_attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           Cfg<64>::kSmemBytes);
+      if (e != cudaSuccess) return e;
+      configured[1] = true;
+    }
+    chunk_attention_kernel<64><<<grid, kThreads, Cfg<64>::kSmemBytes, stream>>>(p);
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace tc

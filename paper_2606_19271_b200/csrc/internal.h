@@ -1,0 +1,82 @@
+// Internal declarations shared by the host-side pool / scheduler and the kernel launchers.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <deque>
+#include <vector>
+
+#include "../../include/turbochunk.h"
+
+namespace tc {
+
+// ---- device-visible schedule records (built per call by the ragged batch scheduler, step a1) ----
+struct SessDesc {      // one per session of the batch
+  int32_t q_off;       // first token of the session in the packed [sum C][H][D] tensors
+  int32_t C;           // chunk tokens
+  int32_t x_begin;     // o + a*T : first visible prior token, in page-table coordinates
+  int32_t x_end;       // o + L   : end of the cached tokens, in page-table coordinates
+  int32_t pt_off;      // offset of this session's page table in the packed page-table array
+  int32_t n_pt;        // pages in the table
+  int32_t pad0, pad1;
+};
+static_assert(sizeof(SessDesc) == 32, "SessDesc layout");
+
+struct WorkItem {      // one (session, head, pair of 128-row query tiles)
+  int32_t sess;        // index into the batch
+  int32_t head;
+  int32_t q_pair;      // query rows [256*q_pair, 256*q_pair + 256) of the session's chunk
+  int32_t n_kv;        // KV tiles of this item (host-computed cost; the kernel recomputes its own loop bounds)
+};
+static_assert(sizeof(WorkItem) == 16, "WorkItem layout");
+
+struct AttnParams {
+  CUtensorMap map_k;             // this layer's cached K: 4D {D, B, H, n_pages}
+  CUtensorMap map_v;             // this layer's cached V
+  const CUtensorMap* sess_maps;  // device [n][3]: per-session Q, Kn, Vn maps (3D {D, H, C_s}); OOB rows zero-fill
+  const SessDesc* sess;
+  const int32_t* page_tables;
+  const WorkItem* items;
+  const int32_t* cta_begin;      // [grid + 1] item ranges per CTA (LPT-balanced on the host)
+  uint16_t* out;                 // bf16 [sum C][H][D]
+  float* lse;                    // fp32 [sum C][H] or null
+  int32_t H, T, B, log2_B;
+  float scale_log2;              // scale * log2(e)
+  float scale;
+};
+
+struct CopySess {      // append / gather descriptor
+  int32_t tok_off;     // first token in the packed source (append) / 0 (gather)
+  int32_t n_tok;       // tokens to copy
+  int32_t n_zero;      // append: trailing slots of the last page to zero-fill after the copied tokens
+  int32_t x0;          // page-table coordinate of the first copied token (o + L for append, o for gather)
+  int32_t pt_off;
+  int32_t row_off;     // cumulative (n_tok + n_zero) rows before this session
+  int32_t pad0, pad1;
+};
+static_assert(sizeof(CopySess) == 32, "CopySess layout");
+
+struct CopyParams {
+  const CopySess* sess;
+  const int32_t* page_tables;
+  int32_t n_sess;
+  int32_t total_rows;       // sum over sessions of (n_tok + n_zero)
+  int32_t H, D, B, log2_B;
+  int64_t page_stride;      // bytes between pages in the slab
+  int64_t layer_k_off;      // byte offset of this layer's K block inside a page
+  int64_t layer_v_off;
+  uint8_t* slab;
+  const uint8_t* src_k;     // append: packed chunk K ; gather: unused
+  const uint8_t* src_v;
+  uint8_t* dst_k;           // gather: logical [L][H][D] output
+  uint8_t* dst_v;
+};
+
+// kernel launchers (return cudaGetLastError())
+cudaError_t launch_attention(const AttnParams& p, int head_dim, int grid, cudaStream_t stream);
+cudaError_t launch_append(const CopyParams& p, int sm_count, cudaStream_t stream);
+cudaError_t launch_gather(const CopyParams& p, int sm_count, cudaStream_t stream);
+int attention_smem_bytes(int head_dim);
+
+}  // namespace tc

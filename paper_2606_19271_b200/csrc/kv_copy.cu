@@ -1,0 +1,113 @@
+// KV append (step a3, PAPER.md:66 (iii) "writes ... updated states back") and logical gather (parity
+// introspection).  Both are pure byte movers: 128-bit vectorised, coalesced on the packed side
+// (contiguous [tokens][H][D]) and in 2*D-byte runs on the paged side ([page][layer][K|V][H][B][D]).
+// HBM-bound: algorithmic bytes = read + write of K and V = 4 * tokens * H * D * 2.
+#include "internal.h"
+
+namespace tc {
+
+constexpr int kCopyThreads = 256;
+constexpr int kCopyUnroll = 4;
+
+__device__ __forceinline__ uint4 ld_stream(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+
+// Byte offset inside the slab (relative to the layer's K or V block of the page) of 16-byte element `e`
+// of a session, where e indexes [row][H][D/8] and row is relative to x0.
+__device__ __forceinline__ int64_t paged_offset(const CopyParams& p, const CopySess& s, const int32_t* pt, int64_t e,
+                                                int vec_per_head, int vec_per_row) {
+  const int row = (int)(e / vec_per_row);
+  const int rem = (int)(e - (int64_t)row * vec_per_row);
+  const int h = rem / vec_per_head;
+  const int v = rem - h * vec_per_head;
+  const int x = s.x0 + row;
+  const int page = pt[x >> p.log2_B];
+  const int slot = x & (p.B - 1);
+  return (int64_t)page * p.page_stride + ((int64_t)h * p.B + slot) * (p.D * 2) + v * 16;
+}
+
+__global__ void __launch_bounds__(kCopyThreads) kv_append_kernel(const CopyParams p) {
+  const CopySess s = p.sess[blockIdx.y];
+  const int32_t* pt = p.page_tables + s.pt_off;
+  const int vec_per_head = p.D / 8;
+  const int vec_per_row = p.H * vec_per_head;
+  const int64_t n_copy = (int64_t)s.n_tok * vec_per_row;
+  const int64_t n_all = (int64_t)(s.n_tok + s.n_zero) * vec_per_row;
+  const uint8_t* src_k = p.src_k + (int64_t)s.tok_off * vec_per_row * 16;
+  const uint8_t* src_v = p.src_v + (int64_t)s.tok_off * vec_per_row * 16;
+  uint8_t* dst_k = p.slab + p.layer_k_off;
+  uint8_t* dst_v = p.slab + p.layer_v_off;
+  const int64_t stride = (int64_t)gridDim.x * kCopyThreads;
+  for (int64_t e0 = (int64_t)blockIdx.x * kCopyThreads + threadIdx.x; e0 < n_all; e0 += stride * kCopyUnroll) {
+    uint4 k[kCopyUnroll], v[kCopyUnroll];
+#pragma unroll
+    for (int u = 0; u < kCopyUnroll; ++u) {
+      const int64_t e = e0 + u * stride;
+      if (e < n_copy) {
+        k[u] = ld_stream(src_k + e * 16);
+        v[u] = ld_stream(src_v + e * 16);
+      } else {
+        k[u] = make_uint4(0, 0, 0, 0);   // zero-fill of the dead tail of the session's last page
+        v[u] = make_uint4(0, 0, 0, 0);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kCopyUnroll; ++u) {
+      const int64_t e = e0 + u * stride;
+      if (e < n_all) {
+        const int64_t off = paged_offset(p, s, pt, e, vec_per_head, vec_per_row);
+        *reinterpret_cast<uint4*>(dst_k + off) = k[u];
+        *reinterpret_cast<uint4*>(dst_v + off) = v[u];
+      }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(kCopyThreads) kv_gather_kernel(const CopyParams p) {
+  const CopySess s = p.sess[blockIdx.y];
+  const int32_t* pt = p.page_tables + s.pt_off;
+  const int vec_per_head = p.D / 8;
+  const int vec_per_row = p.H * vec_per_head;
+  const int64_t n_copy = (int64_t)s.n_tok * vec_per_row;
+  const uint8_t* src_k = p.slab + p.layer_k_off;
+  const uint8_t* src_v = p.slab + p.layer_v_off;
+  uint8_t* dst_k = p.dst_k + (int64_t)s.tok_off * vec_per_row * 16;
+  uint8_t* dst_v = p.dst_v + (int64_t)s.tok_off * vec_per_row * 16;
+  const int64_t stride = (int64_t)gridDim.x * kCopyThreads;
+  for (int64_t e = (int64_t)blockIdx.x * kCopyThreads + threadIdx.x; e < n_copy; e += stride) {
+    const int64_t off = paged_offset(p, s, pt, e, vec_per_head, vec_per_row);
+    const uint4 k = *reinterpret_cast<const uint4*>(src_k + off);
+    const uint4 v = *reinterpret_cast<const uint4*>(src_v + off);
+    *reinterpret_cast<uint4*>(dst_k + e * 16) = k;
+    *reinterpret_cast<uint4*>(dst_v + e * 16) = v;
+  }
+}
+
+static dim3 copy_grid(const CopyParams& p, int sm_count, int64_t max_vecs_per_sess) {
+  // enough CTAs to fill the machine (8 resident CTAs of 256 threads per SM), split evenly over sessions
+  int64_t want = (max_vecs_per_sess + (int64_t)kCopyThreads * kCopyUnroll - 1) / ((int64_t)kCopyThreads * kCopyUnroll);
+  int64_t per_sess_cap = ((int64_t)sm_count * 8 + p.n_sess - 1) / p.n_sess;
+  int64_t gx = want < per_sess_cap ? want : per_sess_cap;
+  if (gx < 1) gx = 1;
+  return dim3((unsigned)gx, (unsigned)p.n_sess, 1);
+}
+
+cudaError_t launch_append(const CopyParams& p, int sm_count, cudaStream_t stream) {
+  // largest per-session element count bounds grid.x; sessions are descriptors on the device, so use the mean
+  const int64_t vec_per_row = (int64_t)p.H * (p.D / 8);
+  const int64_t mean_rows = (p.total_rows + p.n_sess - 1) / p.n_sess;
+  kv_append_kernel<<<copy_grid(p, sm_count, mean_rows * vec_per_row), kCopyThreads, 0, stream>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_gather(const CopyParams& p, int sm_count, cudaStream_t stream) {
+  const int64_t vec_per_row = (int64_t)p.H * (p.D / 8);
+  const int64_t mean_rows = (p.total_rows + p.n_sess - 1) / p.n_sess;
+  kv_gather_kernel<<<copy_grid(p, sm_count, mean_rows * vec_per_row), kCopyThreads, 0, stream>>>(p);
+  return cudaGetLastError();
+}
+
+}  // namespace tc

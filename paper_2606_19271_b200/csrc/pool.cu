@@ -1,0 +1,857 @@
+// Host side of the library: paged KV pool, deterministic FIFO free list, per-session page tables, lifecycle
+// state machine, the ragged batch scheduler (step a1, PAPER.md:66 (i)-(ii)) and the
+// C ABI of include/turbochunk.h.  Device work is launched from here; the kernels live in attention_sm100.cu
+// and kv_copy.cu.
+//
+// Slab layout (private): [page][layer][K|V][H][B][D] bf16.  One page is one contiguous block of
+// NL*2*H*B*D*2 bytes (one cudaMemcpyAsync unit for offload); one (page, layer, K|V, head) block is a dense
+// [B][D] box that TMA loads with a 128-byte swizzle.
+#include <cudaTypedefs.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <queue>
+#include <string>
+
+#include "internal.h"
+
+namespace tc {
+
+static thread_local std::string g_last_cuda_error;
+
+static bool cuda_ok(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return true;
+  g_last_cuda_error = std::string(what) + ": " + cudaGetErrorString(e);
+  cudaGetLastError();   // clear a non-sticky error
+  return false;
+}
+#define TS_CUDA(call)                                  \
+  do {                                                 \
+    if (!tc::cuda_ok((call), #call)) return TS_ERR_CUDA; \
+  } while (0)
+
+static PFN_cuTensorMapEncodeTiled_v12000 get_encode() {
+  static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+  if (fn == nullptr) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(ptr);
+  }
+  return fn;
+}
+
+// Orders work between the caller's compute stream and the pool's side stream without host waits.
+// Every recorded event gets a monotonically increasing sequence number; objects (sessions, pages) remember the
+// sequence number after which they are safe to touch.
+struct EventTimeline {
+  static constexpr uint64_t kRing = 256;
+  cudaEvent_t ev[kRing];
+  uint64_t next_seq = 1;   // 0 means "nothing pending"
+  uint64_t done = 0;       // every seq <= done has completed
+  bool init() {
+    for (uint64_t i = 0; i < kRing; ++i)
+      if (cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming) != cudaSuccess) return false;
+    return true;
+  }
+  void destroy() {
+    for (uint64_t i = 0; i < kRing; ++i) cudaEventDestroy(ev[i]);
+  }
+  bool is_done(uint64_t seq) {
+    while (done < seq && done + 1 < next_seq) {
+      if (cudaEventQuery(ev[(done + 1) % kRing]) == cudaSuccess)
+        ++done;
+      else {
+        cudaGetLastError();
+        break;
+      }
+    }
+    return done >= seq;
+  }
+  uint64_t record(cudaStream_t s) {
+    const uint64_t seq = next_seq++;
+    if (seq > kRing && done < seq - kRing) {   // the slot still belongs to an unfinished older event
+      cudaEventSynchronize(ev[seq % kRing]);
+      done = std::max(done, seq - kRing);
+    }
+    cudaEventRecord(ev[seq % kRing], s);
+    return seq;
+  }
+  cudaError_t wait(cudaStream_t s, uint64_t seq) {
+    if (seq == 0 || is_done(seq)) return cudaSuccess;
+    return cudaStreamWaitEvent(s, ev[seq % kRing], 0);
+  }
+};
+
+struct Session {
+  int state = TS_SESSION_CLOSED;
+  int P = 0;                        // committed cached frames
+  int o = 0;                        // dead slots at the head of the first page
+  std::vector<int32_t> pt;          // physical page ids, logical order
+  std::vector<int32_t> host_slots;  // arena slots holding the pages while SUSPENDED (logical order)
+  uint64_t compute_seq = 0;         // last compute-stream call that touched the session
+  uint64_t side_seq = 0;            // last side-stream copy that touched the session
+};
+
+struct Staging {      // pinned host + device buffer pair for per-call schedule records
+  uint8_t* h = nullptr;
+  uint8_t* d = nullptr;
+  size_t cap = 0;
+  cudaEvent_t ev = nullptr;
+  bool in_flight = false;
+};
+
+}  // namespace tc
+
+using namespace tc;
+
+struct ts_pool {
+  ts_pool_config cfg;
+  int log2_B = 0;
+  int64_t kv_bytes = 0;      // H*B*D*2 : one K (or V) block of one layer of one page
+  int64_t layer_bytes = 0;   // 2*kv_bytes
+  int64_t page_bytes = 0;    // NL*layer_bytes
+  uint8_t* slab = nullptr;
+  bool own_slab = false;
+  uint8_t* host = nullptr;
+  bool own_host = false;
+  int host_pages_cap = 0;
+  std::vector<int32_t> host_free;        // free arena slots (stack)
+  std::deque<int32_t> free_q;            // FIFO free list (R8)
+  std::vector<uint64_t> page_compute_seq, page_side_seq;
+  std::vector<Session> sess;
+  cudaStream_t side = nullptr;
+  bool own_side = false;
+  EventTimeline tl_compute, tl_side;
+  std::vector<CUtensorMap> map_k, map_v;   // per layer
+  int sm_count = 0;
+  static constexpr int kRing = 8;
+  Staging ring[kRing];
+  int ring_next = 0;
+  uint8_t* stage_dev = nullptr;            // ts_chunk_step_host: device staging for q,k,v,out
+  size_t stage_cap = 0;
+  int64_t launches = 0;
+  std::vector<int32_t> scratch_mark;       // duplicate detection
+};
+
+namespace tc {
+
+static bool valid_config(const ts_pool_config* c) {
+  if (c == nullptr) return false;
+  if (c->n_layers < 1 || c->n_heads < 1 || c->n_pages < 1 || c->frame_tokens < 1 || c->max_sessions < 1) return false;
+  if (c->head_dim != 64 && c->head_dim != 128) return false;
+  const int B = c->page_tokens;
+  if (B < 16 || B > 1024 || (B & (B - 1)) != 0) return false;
+  return true;
+}
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static int acquire_staging(ts_pool* pool, size_t bytes, Staging** out) {
+  Staging& s = pool->ring[pool->ring_next];
+  pool->ring_next = (pool->ring_next + 1) % ts_pool::kRing;
+  if (s.ev == nullptr) TS_CUDA(cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming));
+  if (s.in_flight) {
+    TS_CUDA(cudaEventSynchronize(s.ev));   // normally long done: the ring is 8 calls deep
+    s.in_flight = false;
+  }
+  if (s.cap < bytes) {
+    if (s.h) cudaFreeHost(s.h);
+    if (s.d) cudaFree(s.d);
+    s.h = s.d = nullptr;
+    s.cap = 0;
+    const size_t cap = align_up(std::max(bytes * 2, (size_t)65536), 4096);
+    TS_CUDA(cudaHostAlloc((void**)&s.h, cap, cudaHostAllocDefault));
+    TS_CUDA(cudaMalloc((void**)&s.d, cap));
+    s.cap = cap;
+  }
+  *out = &s;
+  return TS_OK;
+}
+
+static int check_batch(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* cf) {
+  const ts_pool_config& c = pool->cfg;
+  if (layer < 0 || layer >= c.n_layers || n < 0) return TS_ERR_INVALID;
+  if (n == 0) return TS_OK;
+  if (sids == nullptr || cf == nullptr) return TS_ERR_INVALID;
+  if (n > c.max_sessions) return TS_ERR_CAPACITY;
+  std::vector<int32_t>& mark = pool->scratch_mark;
+  mark.assign(c.max_sessions, 0);
+  int64_t total = 0;
+  for (int b = 0; b < n; ++b) {
+    if (cf[b] < 1 || (c.window_frames > 0 && cf[b] > c.window_frames)) return TS_ERR_INVALID;
+    total += (int64_t)cf[b] * c.frame_tokens;
+  }
+  if (total > (int64_t)1 << 30) return TS_ERR_INVALID;
+  for (int b = 0; b < n; ++b) {
+    const int sid = sids[b];
+    if (sid < 0 || sid >= c.max_sessions) return TS_ERR_STATE;
+    if (pool->sess[sid].state == TS_SESSION_CLOSED) return TS_ERR_STATE;
+    if (mark[sid]) return TS_ERR_INVALID;
+    mark[sid] = 1;
+  }
+  for (int b = 0; b < n; ++b)
+    if (pool->sess[sids[b]].state != TS_SESSION_RESIDENT) return TS_ERR_STATE;
+  return TS_OK;
+}
+
+static bool encode_map(CUtensorMap* m, void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides,
+                       const cuuint32_t* box) {
+  PFN_cuTensorMapEncodeTiled_v12000 enc = get_encode();
+  if (enc == nullptr) {
+    g_last_cuda_error = "cuTensorMapEncodeTiled entry point not found";
+    return false;
+  }
+  cuuint32_t es[5] = {1, 1, 1, 1, 1};
+  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, rank, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    g_last_cuda_error = "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r);
+    return false;
+  }
+  return true;
+}
+
+// ---- step a1: ragged batch scheduler ---------------------------------------------------------------------
+// Builds, in one pinned staging block: per-session tensor maps, SessDesc, packed page tables, and the work
+// items (session, head, query-tile pair) distributed over `grid` persistent CTAs by longest-processing-time
+// first (cost = KV tiles x query tiles), so that ragged sessions finish together.
+struct ScheduleLayout {
+  size_t off_maps, off_sess, off_pt, off_cta, off_items, bytes;
+  int n_items, grid;
+};
+
+static void item_geometry(const ts_pool_config& c, int C, int x_begin, int x_end, int q_pair, int* n_q, int* n_kv) {
+  const int r0 = q_pair * 256;
+  *n_q = (r0 + 128 < C) ? 2 : 1;
+  const int last_row = std::min(C, r0 + 256) - 1;
+  const int kv_hi = std::min(C, (last_row / c.frame_tokens + 1) * c.frame_tokens);
+  const int n_chunk = (kv_hi + 127) / 128;
+  const int n_prior = x_end > x_begin ? ((x_end - 1) / 128 - x_begin / 128 + 1) : 0;
+  *n_kv = n_prior + n_chunk;
+}
+
+}  // namespace tc
+
+// =================================================================================================== C ABI
+extern "C" {
+
+const char* ts_version(void) { return "turbochunk 0.1 (sm_100a)"; }
+
+const char* ts_strerror(int code) {
+  switch (code) {
+    case TS_OK: return "ok";
+    case TS_ERR_INVALID: return "invalid argument";
+    case TS_ERR_STATE: return "session is in the wrong state";
+    case TS_ERR_NO_PAGES: return "not enough free device pages";
+    case TS_ERR_NO_HOST: return "pinned host arena is full";
+    case TS_ERR_CAPACITY: return "session capacity exceeded";
+    case TS_ERR_CUDA: return "CUDA error";
+    default: return "unknown status";
+  }
+}
+
+const char* ts_last_cuda_error(void) { return tc::g_last_cuda_error.c_str(); }
+
+int64_t ts_pool_page_bytes(const ts_pool_config* cfg) {
+  if (!valid_config(cfg)) return TS_ERR_INVALID;
+  return (int64_t)cfg->n_layers * 2 * cfg->n_heads * cfg->page_tokens * cfg->head_dim * 2;
+}
+
+int64_t ts_pool_slab_bytes(const ts_pool_config* cfg) {
+  if (!valid_config(cfg)) return TS_ERR_INVALID;
+  return ts_pool_page_bytes(cfg) * cfg->n_pages;
+}
+
+int ts_pool_destroy(ts_pool* pool) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  cudaSetDevice(pool->cfg.device);
+  cudaDeviceSynchronize();
+  for (Staging& s : pool->ring) {
+    if (s.h) cudaFreeHost(s.h);
+    if (s.d) cudaFree(s.d);
+    if (s.ev) cudaEventDestroy(s.ev);
+  }
+  if (pool->stage_dev) cudaFree(pool->stage_dev);
+  pool->tl_compute.destroy();
+  pool->tl_side.destroy();
+  if (pool->own_side && pool->side) cudaStreamDestroy(pool->side);
+  if (pool->own_slab && pool->slab) cudaFree(pool->slab);
+  if (pool->own_host && pool->host) cudaFreeHost(pool->host);
+  cudaGetLastError();
+  delete pool;
+  return TS_OK;
+}
+
+int ts_pool_create(const ts_pool_config* cfg, ts_pool** out) {
+  if (out == nullptr) return TS_ERR_INVALID;
+  *out = nullptr;
+  if (!valid_config(cfg)) return TS_ERR_INVALID;
+  if (cfg->free_order != nullptr) {
+    std::vector<char> seen(cfg->n_pages, 0);
+    for (int i = 0; i < cfg->n_pages; ++i) {
+      const int p = cfg->free_order[i];
+      if (p < 0 || p >= cfg->n_pages || seen[p]) return TS_ERR_INVALID;
+      seen[p] = 1;
+    }
+  }
+  const int64_t page_bytes = ts_pool_page_bytes(cfg);
+  const int64_t slab_bytes = page_bytes * cfg->n_pages;
+  if (cfg->kv_slab != nullptr && (cfg->kv_slab_bytes < slab_bytes || ((uintptr_t)cfg->kv_slab & 1023) != 0)) return TS_ERR_INVALID;
+  if (cfg->host_bytes < 0) return TS_ERR_INVALID;
+
+  TS_CUDA(cudaSetDevice(cfg->device));
+  cudaDeviceProp prop;
+  TS_CUDA(cudaGetDeviceProperties(&prop, cfg->device));
+  if (prop.major != 10) {
+    g_last_cuda_error = "device is not sm_100-class (tcgen05/TMEM required); no fallback path exists";
+    return TS_ERR_CUDA;
+  }
+
+  ts_pool* pool = new ts_pool();
+  pool->cfg = *cfg;
+  pool->cfg.free_order = nullptr;
+  pool->sm_count = prop.multiProcessorCount;
+  int l2 = 0;
+  while ((1 << l2) < cfg->page_tokens) ++l2;
+  pool->log2_B = l2;
+  pool->kv_bytes = (int64_t)cfg->n_heads * cfg->page_tokens * cfg->head_dim * 2;
+  pool->layer_bytes = 2 * pool->kv_bytes;
+  pool->page_bytes = page_bytes;
+
+  auto fail = [&](int code) {
+    ts_pool_destroy(pool);
+    return code;
+  };
+  if (!pool->tl_compute.init() || !pool->tl_side.init()) {
+    g_last_cuda_error = "cudaEventCreate failed";
+    return fail(TS_ERR_CUDA);
+  }
+  if (cfg->kv_slab != nullptr) {
+    pool->slab = (uint8_t*)cfg->kv_slab;
+  } else {
+    if (!cuda_ok(cudaMalloc((void**)&pool->slab, slab_bytes), "cudaMalloc(kv slab)")) return fail(TS_ERR_CUDA);
+    pool->own_slab = true;
+  }
+  pool->host_pages_cap = (int)(cfg->host_bytes / page_bytes);
+  if (pool->host_pages_cap > 0) {
+    if (cfg->host_arena != nullptr) {
+      pool->host = (uint8_t*)cfg->host_arena;
+    } else {
+      if (!cuda_ok(cudaHostAlloc((void**)&pool->host, (size_t)pool->host_pages_cap * page_bytes, cudaHostAllocDefault),
+                   "cudaHostAlloc(host arena)"))
+        return fail(TS_ERR_CUDA);
+      pool->own_host = true;
+    }
+  }
+  for (int i = pool->host_pages_cap - 1; i >= 0; --i) pool->host_free.push_back(i);
+  if (cfg->side_stream != nullptr) {
+    pool->side = (cudaStream_t)cfg->side_stream;
+  } else {
+    if (!cuda_ok(cudaStreamCreateWithFlags(&pool->side, cudaStreamNonBlocking), "cudaStreamCreate(side)")) return fail(TS_ERR_CUDA);
+    pool->own_side = true;
+  }
+  for (int i = 0; i < cfg->n_pages; ++i) pool->free_q.push_back(cfg->free_order ? cfg->free_order[i] : i);
+  pool->page_compute_seq.assign(cfg->n_pages, 0);
+  pool->page_side_seq.assign(cfg->n_pages, 0);
+  pool->sess.resize(cfg->max_sessions);
+
+  // per-layer TMA maps of the cached K and V: dims {D, B, H, n_pages}
+  pool->map_k.resize(cfg->n_layers);
+  pool->map_v.resize(cfg->n_layers);
+  const cuuint64_t dims[4] = {(cuuint64_t)cfg->head_dim, (cuuint64_t)cfg->page_tokens, (cuuint64_t)cfg->n_heads,
+                              (cuuint64_t)cfg->n_pages};
+  const cuuint64_t strides[3] = {(cuuint64_t)cfg->head_dim * 2, (cuuint64_t)cfg->page_tokens * cfg->head_dim * 2,
+                                 (cuuint64_t)page_bytes};
+  const cuuint32_t box[4] = {64, (cuuint32_t)std::min(cfg->page_tokens, 128), 1, 1};
+  for (int l = 0; l < cfg->n_layers; ++l) {
+    uint8_t* base = pool->slab + (int64_t)l * pool->layer_bytes;
+    if (!encode_map(&pool->map_k[l], base, 4, dims, strides, box)) return fail(TS_ERR_CUDA);
+    if (!encode_map(&pool->map_v[l], base + pool->kv_bytes, 4, dims, strides, box)) return fail(TS_ERR_CUDA);
+  }
+  *out = pool;
+  return TS_OK;
+}
+
+int ts_session_open(ts_pool* pool, int32_t* sid_out) {
+  if (pool == nullptr || sid_out == nullptr) return TS_ERR_INVALID;
+  for (int i = 0; i < pool->cfg.max_sessions; ++i) {
+    if (pool->sess[i].state == TS_SESSION_CLOSED) {
+      Session& s = pool->sess[i];
+      s = Session();
+      s.state = TS_SESSION_RESIDENT;
+      *sid_out = i;
+      return TS_OK;
+    }
+  }
+  return TS_ERR_CAPACITY;
+}
+
+int ts_session_close(ts_pool* pool, int32_t sid) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  if (sid < 0 || sid >= pool->cfg.max_sessions || pool->sess[sid].state == TS_SESSION_CLOSED) return TS_ERR_STATE;
+  Session& s = pool->sess[sid];
+  if (s.state == TS_SESSION_RESIDENT) {
+    for (int32_t p : s.pt) {
+      pool->page_compute_seq[p] = s.compute_seq;   // in-flight readers/writers of the page
+      pool->page_side_seq[p] = s.side_seq;
+      pool->free_q.push_back(p);
+    }
+  } else {
+    for (auto it = s.host_slots.rbegin(); it != s.host_slots.rend(); ++it) pool->host_free.push_back(*it);
+  }
+  s = Session();
+  return TS_OK;
+}
+
+int ts_session_info(ts_pool* pool, int32_t sid, ts_session_info_t* out) {
+  if (pool == nullptr || out == nullptr) return TS_ERR_INVALID;
+  if (sid < 0 || sid >= pool->cfg.max_sessions || pool->sess[sid].state == TS_SESSION_CLOSED) return TS_ERR_STATE;
+  const Session& s = pool->sess[sid];
+  out->state = s.state;
+  out->frames = s.P;
+  out->len_tokens = (int64_t)s.P * pool->cfg.frame_tokens;
+  out->head_off = s.o;
+  out->n_pages = s.state == TS_SESSION_RESIDENT ? (int32_t)s.pt.size() : (int32_t)s.host_slots.size();
+  return TS_OK;
+}
+
+int ts_session_page_table(ts_pool* pool, int32_t sid, int32_t* out, int32_t cap, int32_t* n_out) {
+  if (pool == nullptr || n_out == nullptr || cap < 0 || (cap > 0 && out == nullptr)) return TS_ERR_INVALID;
+  if (sid < 0 || sid >= pool->cfg.max_sessions || pool->sess[sid].state == TS_SESSION_CLOSED) return TS_ERR_STATE;
+  const Session& s = pool->sess[sid];
+  *n_out = (int32_t)s.pt.size();
+  for (int i = 0; i < std::min<int>(cap, (int)s.pt.size()); ++i) out[i] = s.pt[i];
+  return TS_OK;
+}
+
+int ts_pool_free_list(ts_pool* pool, int32_t* out, int32_t cap, int32_t* n_out) {
+  if (pool == nullptr || n_out == nullptr || cap < 0 || (cap > 0 && out == nullptr)) return TS_ERR_INVALID;
+  *n_out = (int32_t)pool->free_q.size();
+  for (int i = 0; i < std::min<int>(cap, (int)pool->free_q.size()); ++i) out[i] = pool->free_q[i];
+  return TS_OK;
+}
+
+int ts_pool_stats(ts_pool* pool, ts_pool_stats_t* out) {
+  if (pool == nullptr || out == nullptr) return TS_ERR_INVALID;
+  int res = 0, sus = 0;
+  for (const Session& s : pool->sess) {
+    res += s.state == TS_SESSION_RESIDENT;
+    sus += s.state == TS_SESSION_SUSPENDED;
+  }
+  out->free_pages = (int32_t)pool->free_q.size();
+  out->resident = res;
+  out->suspended = sus;
+  out->host_pages_cap = pool->host_pages_cap;
+  out->host_pages_used = pool->host_pages_cap - (int32_t)pool->host_free.size();
+  out->reserved = 0;
+  out->page_bytes = pool->page_bytes;
+  return TS_OK;
+}
+
+void* ts_pool_side_stream(ts_pool* pool) { return pool ? (void*)pool->side : nullptr; }
+int64_t ts_pool_launch_count(ts_pool* pool) { return pool ? pool->launches : 0; }
+
+// --------------------------------------------------------------------------------------------- attention
+int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
+                       const void* q, const void* k, const void* v, void* out, float* lse, float scale, void* cuda_stream) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  int rc = check_batch(pool, layer, n, sids, chunk_frames);
+  if (rc != TS_OK) return rc;
+  if (n == 0) return TS_OK;
+  if (q == nullptr || k == nullptr || v == nullptr || out == nullptr) return TS_ERR_INVALID;
+  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) != 0) return TS_ERR_INVALID;
+  if (!(scale > 0.0f) || !std::isfinite(scale)) return TS_ERR_INVALID;
+  const ts_pool_config& c = pool->cfg;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  TS_CUDA(cudaSetDevice(c.device));
+  const int T = c.frame_tokens, H = c.n_heads, D = c.head_dim, W = c.window_frames;
+
+  // ---- a1: collect + coalesce
+  size_t n_pt_total = 0;
+  int n_items = 0;
+  for (int b = 0; b < n; ++b) {
+    n_pt_total += pool->sess[sids[b]].pt.size();
+    n_items += H * ((chunk_frames[b] * T + 255) / 256);
+  }
+  const int grid = std::min(pool->sm_count, n_items);
+  ScheduleLayout L;
+  L.n_items = n_items;
+  L.grid = grid;
+  L.off_maps = 0;
+  L.off_sess = align_up(L.off_maps + (size_t)n * 3 * sizeof(CUtensorMap), 128);
+  L.off_pt = align_up(L.off_sess + (size_t)n * sizeof(SessDesc), 128);
+  L.off_cta = align_up(L.off_pt + n_pt_total * 4, 128);
+  L.off_items = align_up(L.off_cta + (size_t)(grid + 1) * 4, 128);
+  L.bytes = L.off_items + (size_t)n_items * sizeof(WorkItem);
+  Staging* st = nullptr;
+  rc = acquire_staging(pool, L.bytes, &st);
+  if (rc != TS_OK) return rc;
+  CUtensorMap* maps = reinterpret_cast<CUtensorMap*>(st->h + L.off_maps);
+  SessDesc* sd = reinterpret_cast<SessDesc*>(st->h + L.off_sess);
+  int32_t* pt = reinterpret_cast<int32_t*>(st->h + L.off_pt);
+  int32_t* cta_begin = reinterpret_cast<int32_t*>(st->h + L.off_cta);
+  WorkItem* items = reinterpret_cast<WorkItem*>(st->h + L.off_items);
+
+  struct Cand {
+    int cost, sess, head, q_pair, n_kv;
+  };
+  std::vector<Cand> cands;
+  cands.reserve(n_items);
+  int q_off = 0, pt_off = 0;
+  for (int b = 0; b < n; ++b) {
+    const Session& s = pool->sess[sids[b]];
+    const int cfr = chunk_frames[b];
+    const int C = cfr * T;
+    const int a = W > 0 ? std::max(0, s.P + cfr - W) : 0;     // window start in frames (R6 i)
+    SessDesc& d = sd[b];
+    d.q_off = q_off;
+    d.C = C;
+    d.x_begin = s.o + a * T;
+    d.x_end = s.o + s.P * T;
+    d.pt_off = pt_off;
+    d.n_pt = (int32_t)s.pt.size();
+    d.pad0 = d.pad1 = 0;
+    std::copy(s.pt.begin(), s.pt.end(), pt + pt_off);
+    // per-session 3D maps {D, H, C}: rows past the session's chunk read as zeros, never as a neighbour's tokens
+    const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)H, (cuuint64_t)C};
+    const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)H * D * 2};
+    const cuuint32_t box[3] = {64, 1, 128};
+    const size_t byte_off = (size_t)q_off * H * D * 2;
+    if (!encode_map(&maps[b * 3 + 0], (uint8_t*)q + byte_off, 3, dims, strides, box)) return TS_ERR_CUDA;
+    if (!encode_map(&maps[b * 3 + 1], (uint8_t*)k + byte_off, 3, dims, strides, box)) return TS_ERR_CUDA;
+    if (!encode_map(&maps[b * 3 + 2], (uint8_t*)v + byte_off, 3, dims, strides, box)) return TS_ERR_CUDA;
+    const int n_pairs = (C + 255) / 256;
+    for (int qp = 0; qp < n_pairs; ++qp) {
+      int n_q, n_kv;
+      item_geometry(c, C, d.x_begin, d.x_end, qp, &n_q, &n_kv);
+      const int cost = n_q * (n_kv + 2);      // +2: pipeline fill and epilogue, in KV-tile units
+      for (int h = 0; h < H; ++h) cands.push_back({cost, b, h, qp, n_kv});
+    }
+    q_off += C;
+    pt_off += (int)s.pt.size();
+  }
+  // LPT: heaviest first, each to the least-loaded CTA.  Ties keep (session, head) neighbours adjacent so that
+  // CTAs running concurrently stream the same K/V pages through L2.
+  std::stable_sort(cands.begin(), cands.end(), [](const Cand& x, const Cand& y) { return x.cost > y.cost; });
+  std::vector<std::vector<int>> per_cta(grid);
+  {
+    typedef std::pair<int64_t, int> Load;   // (load, cta)
+    std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
+    for (int i = 0; i < grid; ++i) heap.push({0, i});
+    for (int i = 0; i < (int)cands.size(); ++i) {
+      Load top = heap.top();
+      heap.pop();
+      per_cta[top.second].push_back(i);
+      heap.push({top.first + cands[i].cost, top.second});
+    }
+  }
+  int w = 0;
+  for (int ci = 0; ci < grid; ++ci) {
+    cta_begin[ci] = w;
+    for (int i : per_cta[ci]) {
+      items[w].sess = cands[i].sess;
+      items[w].head = cands[i].head;
+      items[w].q_pair = cands[i].q_pair;
+      items[w].n_kv = cands[i].n_kv;
+      ++w;
+    }
+  }
+  cta_begin[grid] = w;
+
+  // ---- ordering: wait (stream-side) for pending resumes of the batch's sessions
+  for (int b = 0; b < n; ++b) TS_CUDA(pool->tl_side.wait(stream, pool->sess[sids[b]].side_seq));
+
+  TS_CUDA(cudaMemcpyAsync(st->d, st->h, L.bytes, cudaMemcpyHostToDevice, stream));
+  AttnParams p;
+  p.map_k = pool->map_k[layer];
+  p.map_v = pool->map_v[layer];
+  p.sess_maps = reinterpret_cast<const CUtensorMap*>(st->d + L.off_maps);
+  p.sess = reinterpret_cast<const SessDesc*>(st->d + L.off_sess);
+  p.page_tables = reinterpret_cast<const int32_t*>(st->d + L.off_pt);
+  p.cta_begin = reinterpret_cast<const int32_t*>(st->d + L.off_cta);
+  p.items = reinterpret_cast<const WorkItem*>(st->d + L.off_items);
+  p.out = (uint16_t*)out;
+  p.lse = lse;
+  p.H = H;
+  p.T = T;
+  p.B = c.page_tokens;
+  p.log2_B = pool->log2_B;
+  p.scale = scale;
+  p.scale_log2 = scale * 1.4426950408889634f;
+  TS_CUDA(launch_attention(p, D, grid, stream));
+  ++pool->launches;
+  TS_CUDA(cudaEventRecord(st->ev, stream));
+  st->in_flight = true;
+  const uint64_t seq = pool->tl_compute.record(stream);
+  for (int b = 0; b < n; ++b) pool->sess[sids[b]].compute_seq = seq;
+  return TS_OK;
+}
+
+// --------------------------------------------------------------------------------------------- append
+int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames, const void* k,
+                 const void* v, uint32_t flags, void* cuda_stream) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  int rc = check_batch(pool, layer, n, sids, chunk_frames);
+  if (rc != TS_OK) return rc;
+  if (n == 0) return TS_OK;
+  if (k == nullptr || v == nullptr || (((uintptr_t)k | (uintptr_t)v) & 15) != 0) return TS_ERR_INVALID;
+  if ((flags & ~(uint32_t)TS_COMMIT) != 0) return TS_ERR_INVALID;
+  const ts_pool_config& c = pool->cfg;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  TS_CUDA(cudaSetDevice(c.device));
+  const int T = c.frame_tokens, B = c.page_tokens, W = c.window_frames;
+
+  // demand check first: all-or-nothing (O2)
+  std::vector<int> need(n);
+  int64_t need_total = 0;
+  size_t n_pt_total = 0;
+  for (int b = 0; b < n; ++b) {
+    const Session& s = pool->sess[sids[b]];
+    const int64_t end = (int64_t)s.o + (int64_t)s.P * T + (int64_t)chunk_frames[b] * T;
+    need[b] = (int)((end + B - 1) / B) - (int)s.pt.size();
+    if (need[b] < 0) need[b] = 0;
+    need_total += need[b];
+    n_pt_total += s.pt.size() + need[b];
+  }
+  if (need_total > (int64_t)pool->free_q.size()) return TS_ERR_NO_PAGES;
+
+  const size_t off_sess = 0;
+  const size_t off_pt = align_up((size_t)n * sizeof(CopySess), 128);
+  const size_t bytes = off_pt + n_pt_total * 4;
+  Staging* st = nullptr;
+  rc = acquire_staging(pool, bytes, &st);
+  if (rc != TS_OK) return rc;
+  CopySess* cs = reinterpret_cast<CopySess*>(st->h + off_sess);
+  int32_t* pt = reinterpret_cast<int32_t*>(st->h + off_pt);
+
+  uint64_t wait_side = 0, wait_compute = 0;
+  int tok_off = 0, pt_off = 0, row_off = 0;
+  for (int b = 0; b < n; ++b) {
+    Session& s = pool->sess[sids[b]];
+    for (int i = 0; i < need[b]; ++i) {
+      const int32_t pg = pool->free_q.front();
+      pool->free_q.pop_front();
+      wait_side = std::max(wait_side, pool->page_side_seq[pg]);        // a D2H copy out of the page may be pending
+      wait_compute = std::max(wait_compute, pool->page_compute_seq[pg]);
+      s.pt.push_back(pg);
+    }
+    wait_side = std::max(wait_side, s.side_seq);
+    const int C = chunk_frames[b] * T;
+    const int x0 = s.o + s.P * T;
+    CopySess& d = cs[b];
+    d.tok_off = tok_off;
+    d.n_tok = C;
+    d.n_zero = (B - ((x0 + C) & (B - 1))) & (B - 1);
+    d.x0 = x0;
+    d.pt_off = pt_off;
+    d.row_off = row_off;
+    d.pad0 = d.pad1 = 0;
+    std::copy(s.pt.begin(), s.pt.end(), pt + pt_off);
+    tok_off += C;
+    pt_off += (int)s.pt.size();
+    row_off += d.n_tok + d.n_zero;
+  }
+  TS_CUDA(pool->tl_side.wait(stream, wait_side));
+  TS_CUDA(pool->tl_compute.wait(stream, wait_compute));
+  TS_CUDA(cudaMemcpyAsync(st->d, st->h, bytes, cudaMemcpyHostToDevice, stream));
+  CopyParams p;
+  memset(&p, 0, sizeof(p));
+  p.sess = reinterpret_cast<const CopySess*>(st->d + off_sess);
+  p.page_tables = reinterpret_cast<const int32_t*>(st->d + off_pt);
+  p.n_sess = n;
+  p.total_rows = row_off;
+  p.H = c.n_heads;
+  p.D = c.head_dim;
+  p.B = B;
+  p.log2_B = pool->log2_B;
+  p.page_stride = pool->page_bytes;
+  p.layer_k_off = (int64_t)layer * pool->layer_bytes;
+  p.layer_v_off = p.layer_k_off + pool->kv_bytes;
+  p.slab = pool->slab;
+  p.src_k = (const uint8_t*)k;
+  p.src_v = (const uint8_t*)v;
+  TS_CUDA(launch_append(p, pool->sm_count, stream));
+  ++pool->launches;
+  TS_CUDA(cudaEventRecord(st->ev, stream));
+  st->in_flight = true;
+  const uint64_t seq = pool->tl_compute.record(stream);
+
+  for (int b = 0; b < n; ++b) {
+    Session& s = pool->sess[sids[b]];
+    s.compute_seq = seq;
+    if (flags & TS_COMMIT) {
+      s.P += chunk_frames[b];
+      const int e = W > 0 ? std::max(0, s.P - W) : 0;   // a4: evict oldest whole frames (R6 ii, R10)
+      s.P -= e;
+      s.o += e * T;
+      while (s.o >= B) {
+        const int32_t pg = s.pt.front();
+        s.pt.erase(s.pt.begin());
+        pool->page_compute_seq[pg] = seq;
+        pool->page_side_seq[pg] = s.side_seq;
+        pool->free_q.push_back(pg);
+        s.o -= B;
+      }
+    }
+  }
+  return TS_OK;
+}
+
+// --------------------------------------------------------------------------------------------- gather
+int ts_gather_kv(ts_pool* pool, int32_t layer, int32_t sid, void* k_out, void* v_out, void* cuda_stream) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  const ts_pool_config& c = pool->cfg;
+  if (layer < 0 || layer >= c.n_layers) return TS_ERR_INVALID;
+  if (sid < 0 || sid >= c.max_sessions || pool->sess[sid].state != TS_SESSION_RESIDENT) return TS_ERR_STATE;
+  Session& s = pool->sess[sid];
+  const int L = s.P * c.frame_tokens;
+  if (L == 0) return TS_OK;
+  if (k_out == nullptr || v_out == nullptr || (((uintptr_t)k_out | (uintptr_t)v_out) & 15) != 0) return TS_ERR_INVALID;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  TS_CUDA(cudaSetDevice(c.device));
+  const size_t off_pt = 128;
+  const size_t bytes = off_pt + s.pt.size() * 4;
+  Staging* st = nullptr;
+  int rc = acquire_staging(pool, bytes, &st);
+  if (rc != TS_OK) return rc;
+  CopySess* cs = reinterpret_cast<CopySess*>(st->h);
+  cs->tok_off = 0;
+  cs->n_tok = L;
+  cs->n_zero = 0;
+  cs->x0 = s.o;
+  cs->pt_off = 0;
+  cs->row_off = 0;
+  cs->pad0 = cs->pad1 = 0;
+  std::copy(s.pt.begin(), s.pt.end(), reinterpret_cast<int32_t*>(st->h + off_pt));
+  TS_CUDA(pool->tl_side.wait(stream, s.side_seq));
+  TS_CUDA(cudaMemcpyAsync(st->d, st->h, bytes, cudaMemcpyHostToDevice, stream));
+  CopyParams p;
+  memset(&p, 0, sizeof(p));
+  p.sess = reinterpret_cast<const CopySess*>(st->d);
+  p.page_tables = reinterpret_cast<const int32_t*>(st->d + off_pt);
+  p.n_sess = 1;
+  p.total_rows = L;
+  p.H = c.n_heads;
+  p.D = c.head_dim;
+  p.B = c.page_tokens;
+  p.log2_B = pool->log2_B;
+  p.page_stride = pool->page_bytes;
+  p.layer_k_off = (int64_t)layer * pool->layer_bytes;
+  p.layer_v_off = p.layer_k_off + pool->kv_bytes;
+  p.slab = pool->slab;
+  p.dst_k = (uint8_t*)k_out;
+  p.dst_v = (uint8_t*)v_out;
+  TS_CUDA(launch_gather(p, pool->sm_count, stream));
+  ++pool->launches;
+  TS_CUDA(cudaEventRecord(st->ev, stream));
+  st->in_flight = true;
+  s.compute_seq = pool->tl_compute.record(stream);
+  return TS_OK;
+}
+
+// --------------------------------------------------------------------------------------------- offload
+int ts_session_suspend(ts_pool* pool, int32_t sid) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  const ts_pool_config& c = pool->cfg;
+  if (sid < 0 || sid >= c.max_sessions || pool->sess[sid].state != TS_SESSION_RESIDENT) return TS_ERR_STATE;
+  Session& s = pool->sess[sid];
+  if (s.pt.size() > pool->host_free.size()) return TS_ERR_NO_HOST;
+  TS_CUDA(cudaSetDevice(c.device));
+  // chunk-boundary rule (R12): the copy out starts after the compute work already enqueued on the session
+  TS_CUDA(pool->tl_compute.wait(pool->side, s.compute_seq));
+  s.host_slots.clear();
+  for (size_t i = 0; i < s.pt.size(); ++i) {
+    const int32_t slot = pool->host_free.back();
+    pool->host_free.pop_back();
+    s.host_slots.push_back(slot);
+    TS_CUDA(cudaMemcpyAsync(pool->host + (int64_t)slot * pool->page_bytes, pool->slab + (int64_t)s.pt[i] * pool->page_bytes,
+                            pool->page_bytes, cudaMemcpyDeviceToHost, pool->side));
+  }
+  const uint64_t seq = pool->tl_side.record(pool->side);
+  for (int32_t pg : s.pt) {
+    pool->page_side_seq[pg] = seq;
+    pool->page_compute_seq[pg] = s.compute_seq;
+    pool->free_q.push_back(pg);
+  }
+  s.pt.clear();
+  s.side_seq = seq;
+  s.state = TS_SESSION_SUSPENDED;
+  return TS_OK;
+}
+
+int ts_session_resume(ts_pool* pool, int32_t sid) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  const ts_pool_config& c = pool->cfg;
+  if (sid < 0 || sid >= c.max_sessions || pool->sess[sid].state != TS_SESSION_SUSPENDED) return TS_ERR_STATE;
+  Session& s = pool->sess[sid];
+  if (s.host_slots.size() > pool->free_q.size()) return TS_ERR_NO_PAGES;
+  TS_CUDA(cudaSetDevice(c.device));
+  uint64_t wait_compute = 0;
+  for (size_t i = 0; i < s.host_slots.size(); ++i) {
+    const int32_t pg = pool->free_q.front();
+    pool->free_q.pop_front();
+    wait_compute = std::max(wait_compute, pool->page_compute_seq[pg]);   // readers of the page's previous owner
+    s.pt.push_back(pg);
+  }
+  TS_CUDA(pool->tl_compute.wait(pool->side, wait_compute));
+  for (size_t i = 0; i < s.pt.size(); ++i) {
+    TS_CUDA(cudaMemcpyAsync(pool->slab + (int64_t)s.pt[i] * pool->page_bytes, pool->host + (int64_t)s.host_slots[i] * pool->page_bytes,
+                            pool->page_bytes, cudaMemcpyHostToDevice, pool->side));
+  }
+  s.side_seq = pool->tl_side.record(pool->side);
+  for (auto it = s.host_slots.rbegin(); it != s.host_slots.rend(); ++it) pool->host_free.push_back(*it);
+  s.host_slots.clear();
+  s.state = TS_SESSION_RESIDENT;
+  return TS_OK;
+}
+
+int ts_offload_sync(ts_pool* pool) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  TS_CUDA(cudaSetDevice(pool->cfg.device));
+  TS_CUDA(cudaStreamSynchronize(pool->side));
+  return TS_OK;
+}
+
+// --------------------------------------------------------------------------------------------- host-buffer step
+int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
+                       const void* q_host, const void* k_host, const void* v_host, void* out_host, float scale, uint32_t flags,
+                       void* cuda_stream) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  int rc = check_batch(pool, layer, n, sids, chunk_frames);
+  if (rc != TS_OK) return rc;
+  if (n == 0) return TS_OK;
+  if (q_host == nullptr || k_host == nullptr || v_host == nullptr || out_host == nullptr) return TS_ERR_INVALID;
+  const ts_pool_config& c = pool->cfg;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  TS_CUDA(cudaSetDevice(c.device));
+  int64_t tokens = 0;
+  for (int b = 0; b < n; ++b) tokens += (int64_t)chunk_frames[b] * c.frame_tokens;
+  const size_t tensor_bytes = align_up((size_t)tokens * c.n_heads * c.head_dim * 2, 1024);
+  if (pool->stage_cap < 4 * tensor_bytes) {
+    if (pool->stage_dev) {
+      TS_CUDA(cudaDeviceSynchronize());
+      TS_CUDA(cudaFree(pool->stage_dev));
+      pool->stage_dev = nullptr;
+      pool->stage_cap = 0;
+    }
+    TS_CUDA(cudaMalloc((void**)&pool->stage_dev, 4 * tensor_bytes));
+    pool->stage_cap = 4 * tensor_bytes;
+  }
+  uint8_t* dq = pool->stage_dev;
+  uint8_t* dk = dq + tensor_bytes;
+  uint8_t* dv = dk + tensor_bytes;
+  uint8_t* dout = dv + tensor_bytes;
+  const size_t nbytes = (size_t)tokens * c.n_heads * c.head_dim * 2;
+  TS_CUDA(cudaMemcpyAsync(dq, q_host, nbytes, cudaMemcpyHostToDevice, stream));
+  TS_CUDA(cudaMemcpyAsync(dk, k_host, nbytes, cudaMemcpyHostToDevice, stream));
+  TS_CUDA(cudaMemcpyAsync(dv, v_host, nbytes, cudaMemcpyHostToDevice, stream));
+  rc = ts_chunk_attention(pool, layer, n, sids, chunk_frames, dq, dk, dv, dout, nullptr, scale, cuda_stream);
+  if (rc != TS_OK) return rc;
+  TS_CUDA(cudaMemcpyAsync(out_host, dout, nbytes, cudaMemcpyDeviceToHost, stream));
+  return ts_kv_append(pool, layer, n, sids, chunk_frames, dk, dv, flags, cuda_stream);
+}
+
+}  // extern "C"
