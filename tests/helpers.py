@@ -40,3 +40,108 @@ def build_oracle_workload(w):
 
 def rel_l2(a, b):
     return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# GPU-side helpers (imported lazily so that the CPU-only tests never touch the CUDA binding)
+# ---------------------------------------------------------------------------------------------------------
+def bits_to_dev(bits, device="cuda"):
+    """uint16 bf16 bit patterns (numpy) -> torch bf16 tensor on the device (no value change)."""
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).to(device).view(torch.bfloat16)
+
+
+def dev_to_bits(t):
+    """torch bf16 tensor -> numpy uint16 bit patterns."""
+    import torch
+    return t.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+class DualPool:
+    """Drives the oracle pool and the CUDA pool with the same operations and compares what is unique:
+    page tables, free list, (len, head_off, n_pages), logical KV bytes (bit-exact) and attention output
+    (max-abs <= 2e-2, rel-L2 <= 5e-3 against fp64 — BASELINE.json north_star)."""
+
+    MAX_ABS, REL_L2 = 2e-2, 5e-3
+
+    def __init__(self, shape, free_order=None, host_pages=0):
+        from paper_2606_19271_b200 import TurboChunkPool
+        self.shape = shape
+        self.o = make_oracle_pool(shape, free_order, host_pages if host_pages else None)
+        self.g = TurboChunkPool(shape.n_layers, shape.n_heads, shape.head_dim, shape.page_tokens, shape.n_pages,
+                                shape.frame_tokens, shape.window_frames, shape.max_sessions,
+                                free_order=free_order, host_pages=host_pages)
+
+    def open(self):
+        a, b = self.o.open(), self.g.ts_session_open()
+        assert a == b
+        return a
+
+    def close(self, sid):
+        self.o.close(sid)
+        self.g.ts_session_close(sid)
+
+    def append(self, layer, sids, cf, k_bits, v_bits, commit=True, dev=None):
+        from paper_2606_19271_b200 import TS_COMMIT
+        self.o.append(layer, sids, cf, k_bits, v_bits, commit=commit)
+        dk, dv = dev if dev is not None else (bits_to_dev(k_bits), bits_to_dev(v_bits))
+        self.g.ts_kv_append(layer, sids, cf, dk, dv, TS_COMMIT if commit else 0)
+
+    def feed_prior(self, sid, k_layers, v_layers, frames_per_append=3):
+        T = self.shape.frame_tokens
+        n_frames = k_layers[0].shape[0] // T
+        f = 0
+        while f < n_frames:
+            c = min(frames_per_append, n_frames - f)
+            lo, hi = f * T, (f + c) * T
+            for layer in range(len(k_layers)):
+                self.append(layer, [sid], [c], k_layers[layer][lo:hi], v_layers[layer][lo:hi],
+                            commit=(layer == len(k_layers) - 1))
+            f += c
+
+    def suspend(self, sid):
+        self.o.suspend(sid)
+        self.g.ts_session_suspend(sid)
+
+    def resume(self, sid):
+        self.o.resume(sid)
+        self.g.ts_session_resume(sid)
+
+    def attention(self, layer, sids, cf, q_bits, k_bits, v_bits, scale, check=True, with_lse=True):
+        import torch
+        o_ref, lse_ref = oracle.chunk_attention(self.o, layer, sids, cf, q_bits, k_bits, v_bits, scale)
+        dq, dk, dv = bits_to_dev(q_bits), bits_to_dev(k_bits), bits_to_dev(v_bits)
+        out = torch.full_like(dq, float("nan"))
+        lse = torch.full(dq.shape[:2], float("nan"), dtype=torch.float32, device=dq.device) if with_lse else None
+        self.g.ts_chunk_attention(layer, sids, cf, dq, dk, dv, out, lse, float(scale))
+        torch.cuda.synchronize()
+        o_gpu = out.double().cpu().numpy()
+        if check:
+            assert np.isfinite(o_gpu).all()
+            max_abs = float(np.abs(o_gpu - o_ref).max())
+            rl2 = rel_l2(o_gpu, o_ref)
+            assert max_abs <= self.MAX_ABS and rl2 <= self.REL_L2, (max_abs, rl2)
+            if with_lse:
+                l_gpu = lse.double().cpu().numpy()
+                assert np.abs(l_gpu - lse_ref).max() <= 2e-3, float(np.abs(l_gpu - lse_ref).max())
+        return o_gpu, o_ref
+
+    def check_state(self, sids, layers=None, kv=True):
+        import torch
+        assert list(self.o.free) == self.g.ts_pool_free_list()
+        st_o, st_g = self.o.stats(), self.g.ts_pool_stats()
+        for key in ("free_pages", "resident", "suspended", "host_pages_used"):
+            assert st_o[key] == st_g[key], (key, st_o, st_g)
+        for sid in sids:
+            io, ig = self.o.info(sid), self.g.ts_session_info(sid)
+            assert ig["state"] == (1 if io["state"] == oracle.RESIDENT else 2)
+            for key in ("frames", "len_tokens", "head_off", "n_pages"):
+                assert io[key] == ig[key], (sid, key, io, ig)
+            assert self.o.page_table(sid) == self.g.ts_session_page_table(sid)
+            if kv and io["state"] == oracle.RESIDENT:
+                for layer in (layers if layers is not None else range(self.shape.n_layers)):
+                    gk, gv = self.g.ts_gather_kv(layer, sid)
+                    torch.cuda.synchronize()
+                    ok, ov = self.o.gather_kv(layer, sid)
+                    assert np.array_equal(dev_to_bits(gk), ok), f"K bytes differ sid={sid} layer={layer}"
+                    assert np.array_equal(dev_to_bits(gv), ov), f"V bytes differ sid={sid} layer={layer}"

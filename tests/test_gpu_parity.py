@@ -1,0 +1,309 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+Integer / byte work is bit-exact; attention is within max-abs 2e-2 and rel-L2 5e-3 of fp64
+(BASELINE.json north_star)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from helpers import DualPool, bits_to_dev, dev_to_bits, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+def shape_of(**kw):
+    d = dict(n_layers=1, n_heads=2, head_dim=128, page_tokens=256, n_pages=64, frame_tokens=200,
+             window_frames=0, max_sessions=8)
+    d.update(kw)
+    return synth.PoolShape(**d)
+
+
+def draw(rng, n, shape):
+    return synth.draw_bits(rng, n, shape.n_heads, shape.head_dim)
+
+
+def scale_of(shape):
+    return np.float32(1.0 / np.sqrt(np.float32(shape.head_dim)))
+
+
+# ---- configs[0]: Tiny, the whole sequence of BASELINE.json --------------------------------------------------
+def test_config0_tiny_full_sequence():
+    w = synth.tiny()
+    dp = DualPool(w.shape, w.free_order, host_pages=8)
+    sids = [dp.open() for _ in w.sessions]
+    tensors = [synth.draw_session_tensors(w.rng, w.shape, s) for s in w.sessions]
+    dp.feed_prior(sids[1], tensors[1]["prior_k"], tensors[1]["prior_v"])
+    dp.check_state(sids)
+    q, k, v = (np.concatenate([t[n] for t in tensors]) for n in ("q", "k", "v"))
+    cf = [s.chunk_frames for s in w.sessions]
+    dp.attention(0, sids, cf, q, k, v, w.scale)
+    dp.append(0, sids, cf, k, v)
+    dp.check_state(sids)
+    dp.suspend(sids[1])
+    dp.check_state(sids)
+    dp.resume(sids[1])
+    dp.check_state(sids)
+    assert dp.g.ts_session_page_table(sids[1]) == [5, 14, 12, 6, 9]       # tests/golden/tiny_allocator_trace.txt
+    dp.attention(0, sids, [1, 1], q[:32], k[:32], v[:32], w.scale)        # after the round trip
+
+
+# ---- configs[1]: Wan-1.3B-shaped single session, full oracle ------------------------------------------------
+def test_config1_wan13b_single():
+    w = synth.wan13b_single()
+    dp = DualPool(w.shape, w.free_order)
+    sid = dp.open()
+    t = synth.draw_session_tensors(w.rng, w.shape, w.sessions[0])
+    dp.feed_prior(sid, t["prior_k"], t["prior_v"])
+    dp.check_state([sid])
+    o_gpu, o_ref = dp.attention(0, [sid], [3], t["q"], t["k"], t["v"], w.scale)
+    # P12: output std ~ sqrt(e/n) for the last frame's rows
+    n = 9 * 1560
+    assert abs(o_gpu[2 * 1560:].std() / np.sqrt(np.e / n) - 1) < 0.1
+    dp.append(0, [sid], [3], t["k"], t["v"])
+    dp.check_state([sid])
+
+
+# ---- ragged coalesced batch: different priors, window clamp, evicted head offset, T not a multiple of 128 --
+@pytest.mark.parametrize("head_dim,page_tokens", [(128, 256), (64, 256), (128, 64), (64, 16), (128, 1024)])
+def test_ragged_batch_window_and_offsets(head_dim, page_tokens):
+    shape = shape_of(head_dim=head_dim, page_tokens=page_tokens, n_heads=3, frame_tokens=203, window_frames=7,
+                     n_pages=max(64, 8 * 1800 // page_tokens), max_sessions=8)
+    rng = np.random.default_rng(100 + head_dim + page_tokens)
+    dp = DualPool(shape, rng.permutation(shape.n_pages), host_pages=shape.n_pages)
+    T = shape.frame_tokens
+    priors = [0, 2, 5, 7, 11]            # 7 and 11 frames: window is full / has rolled (head offset != 0)
+    chunks = [3, 1, 2, 3, 3]
+    sids = [dp.open() for _ in priors]
+    for sid, P in zip(sids, priors):
+        if P:
+            dp.feed_prior(sid, [draw(rng, P * T, shape)], [draw(rng, P * T, shape)])
+    assert dp.g.ts_session_info(sids[4])["head_off"] != 0
+    dp.check_state(sids)
+    total = sum(chunks) * T
+    q, k, v = (draw(rng, total, shape) for _ in range(3))
+    dp.attention(0, sids, chunks, q, k, v, scale_of(shape))
+    dp.append(0, sids, chunks, k, v)
+    dp.check_state(sids)
+    # suspend two sessions, run the rest, resume, run all again (event ordering across streams)
+    dp.suspend(sids[2])
+    dp.suspend(sids[4])
+    rest = [sids[0], sids[1], sids[3]]
+    q2, k2, v2 = (draw(rng, 3 * T, shape) for _ in range(3))
+    dp.attention(0, rest, [1, 1, 1], q2, k2, v2, scale_of(shape))
+    dp.resume(sids[4])
+    dp.resume(sids[2])
+    dp.check_state(sids)
+    dp.attention(0, sids, chunks, q, k, v, scale_of(shape))
+
+
+# ---- small / degenerate shapes ------------------------------------------------------------------------------
+@pytest.mark.parametrize("frame_tokens,chunk,prior", [(1, 5, 0), (1, 1, 0), (7, 1, 0), (128, 2, 1), (129, 3, 2),
+                                                       (100, 1, 0), (300, 1, 3), (257, 2, 0)])
+def test_degenerate_shapes(frame_tokens, chunk, prior):
+    shape = shape_of(frame_tokens=frame_tokens, page_tokens=32, n_pages=128)
+    rng = np.random.default_rng(7 * frame_tokens + chunk)
+    dp = DualPool(shape, rng.permutation(shape.n_pages))
+    sid = dp.open()
+    T = frame_tokens
+    if prior:
+        dp.feed_prior(sid, [draw(rng, prior * T, shape)], [draw(rng, prior * T, shape)])
+    q, k, v = (draw(rng, chunk * T, shape) for _ in range(3))
+    dp.attention(0, [sid], [chunk], q, k, v, np.float32(0.11))
+    dp.append(0, [sid], [chunk], k, v)
+    dp.check_state([sid])
+
+
+def test_single_visible_key_and_constant_v_on_gpu():
+    shape = shape_of(frame_tokens=1, page_tokens=16, n_pages=16)
+    rng = np.random.default_rng(5)
+    dp = DualPool(shape)
+    sid = dp.open()
+    q, k, v = (draw(rng, 4, shape) for _ in range(3))
+    o_gpu, _ = dp.attention(0, [sid], [4], q, k, v, np.float32(0.3))
+    np.testing.assert_array_equal(o_gpu[0], synth.bf16_bits_to_f64(v)[0])          # P3: exactly v_0
+    u = draw(rng, 1, shape)
+    vc = np.repeat(u, 4, axis=0)
+    o_gpu, _ = dp.attention(0, [sid], [4], q, k, vc, np.float32(0.3))
+    np.testing.assert_allclose(o_gpu, np.broadcast_to(synth.bf16_bits_to_f64(u), o_gpu.shape), rtol=2 ** -8)
+
+
+# ---- multi-layer step (configs[3]-shaped, scaled down): growth once, commit on the last layer --------------
+def test_multilayer_commit_on_last_layer():
+    shape = shape_of(n_layers=3, n_heads=5, frame_tokens=150, window_frames=6, n_pages=64, page_tokens=128)
+    rng = np.random.default_rng(9)
+    dp = DualPool(shape, rng.permutation(shape.n_pages), host_pages=40)
+    T = shape.frame_tokens
+    sids = [dp.open(), dp.open()]
+    for step in range(3):                      # 3 chunk steps of 3 frames: window (6) rolls on the third
+        qs = [draw(rng, 6 * T, shape) for _ in range(3)]
+        ks = [draw(rng, 6 * T, shape) for _ in range(3)]
+        vs = [draw(rng, 6 * T, shape) for _ in range(3)]
+        for layer in range(3):
+            dp.attention(layer, sids, [3, 3], qs[layer], ks[layer], vs[layer], scale_of(shape))
+            dp.append(layer, sids, [3, 3], ks[layer], vs[layer], commit=(layer == 2))
+        dp.check_state(sids)
+    dp.suspend(sids[0])
+    dp.check_state(sids)
+    dp.resume(sids[0])
+    dp.check_state(sids)
+
+
+# ---- batch-composition invariance on the GPU: bitwise ------------------------------------------------------
+def test_gpu_batch_composition_invariance():
+    shape = shape_of(n_heads=2, frame_tokens=180, window_frames=9, page_tokens=64, n_pages=256)
+    rng = np.random.default_rng(11)
+    T = shape.frame_tokens
+    priors = {0: 4, 1: 0, 2: 6}
+    pk = {s: draw(rng, P * T, shape) for s, P in priors.items()}
+    pv = {s: draw(rng, P * T, shape) for s, P in priors.items()}
+    ch = {s: tuple(draw(rng, 3 * T, shape) for _ in range(3)) for s in priors}
+
+    def run(order):
+        dp = DualPool(shape, np.random.default_rng(1).permutation(shape.n_pages))
+        sid = {s: dp.open() for s in order}
+        for s in order:
+            if priors[s]:
+                dp.feed_prior(sid[s], [pk[s]], [pv[s]])
+        q, k, v = (np.concatenate([ch[s][i] for s in order]) for i in range(3))
+        dq, dk, dv = bits_to_dev(q), bits_to_dev(k), bits_to_dev(v)
+        out = torch.empty_like(dq)
+        dp.g.ts_chunk_attention(0, [sid[s] for s in order], [3] * len(order), dq, dk, dv, out, None, 0.09)
+        torch.cuda.synchronize()
+        bits = dev_to_bits(out)
+        return {s: bits[i * 3 * T:(i + 1) * 3 * T] for i, s in enumerate(order)}
+
+    full = run([0, 1, 2])
+    for order in ([2, 1, 0], [1], [0, 2]):
+        part = run(order)
+        for s in order:
+            np.testing.assert_array_equal(part[s], full[s])
+
+
+# ---- error behaviour through the ABI ---------------------------------------------------------------------------
+def test_error_codes_and_all_or_nothing():
+    import paper_2606_19271_b200 as tc
+    shape = shape_of(n_pages=8, max_sessions=2, window_frames=4, frame_tokens=100, page_tokens=64)
+    rng = np.random.default_rng(13)
+    dp = DualPool(shape, host_pages=2)
+    a, b = dp.open(), dp.open()
+    with pytest.raises(tc.TurboChunkError) as e:
+        dp.g.ts_session_open()
+    assert e.value.code == tc.TS_ERR_CAPACITY
+    k1 = bits_to_dev(draw(rng, 200, shape))
+    with pytest.raises(tc.TurboChunkError) as e:
+        dp.g.ts_kv_append(0, [a, a], [1, 1], k1, k1)
+    assert e.value.code == tc.TS_ERR_INVALID
+    with pytest.raises(tc.TurboChunkError) as e:
+        dp.g.ts_kv_append(0, [a], [5], k1, k1)
+    assert e.value.code == tc.TS_ERR_INVALID
+    with pytest.raises(tc.TurboChunkError) as e:
+        dp.g.ts_kv_append(3, [a], [1], k1, k1)
+    assert e.value.code == tc.TS_ERR_INVALID
+    big = draw(rng, 400, shape)
+    dp.append(0, [a], [4], big, big)                       # 400 tokens = 7 pages of 64
+    free_before = dp.g.ts_pool_free_list()
+    with pytest.raises(tc.TurboChunkError) as e:           # needs 2 pages, 1 free
+        dp.g.ts_kv_append(0, [b], [1], k1, k1)
+    assert e.value.code == tc.TS_ERR_NO_PAGES
+    with pytest.raises(oracle.OracleError) as eo:
+        dp.o.append(0, [b], [1], big[:100], big[:100])
+    assert eo.value.kind == oracle.NO_PAGES
+    assert dp.g.ts_pool_free_list() == free_before and dp.g.ts_session_page_table(b) == []
+    with pytest.raises(tc.TurboChunkError) as e:
+        dp.g.ts_session_suspend(a)                         # 7 pages > 2 host pages
+    assert e.value.code == tc.TS_ERR_NO_HOST
+    with pytest.raises(tc.TurboChunkError) as e:
+        dp.g.ts_session_resume(a)
+    assert e.value.code == tc.TS_ERR_STATE
+    q = bits_to_dev(draw(rng, 100, shape))
+    out = torch.empty_like(q)
+    with pytest.raises(tc.TurboChunkError) as e:
+        dp.g.ts_chunk_attention(0, [a], [1], q, q, q, out, None, -1.0)
+    assert e.value.code == tc.TS_ERR_INVALID
+    dp.g.ts_chunk_attention(0, [], [], None, None, None, None, None, 1.0)     # n == 0: no-op
+    dp.g.ts_kv_append(0, [], [], None, None)
+    dp.close(a)
+    dp.check_state([b])
+    with pytest.raises(tc.TurboChunkError) as e:
+        dp.g.ts_session_close(a)
+    assert e.value.code == tc.TS_ERR_STATE
+    assert dp.open() == a
+
+
+# ---- configs[4]-style churn, scaled down: integers at every step, KV bytes and attention sampled -----------
+def test_churn_scaled_down():
+    shape = shape_of(n_heads=2, head_dim=128, frame_tokens=40, window_frames=9, page_tokens=16,
+                     n_pages=12 * 36, max_sessions=40)
+    steps = synth.churn_script(seed=4, n_steps=60, cap=12, mean_off=2.0, mean_on=9.0)
+    rng = np.random.default_rng(4)
+    dp = DualPool(shape, rng.permutation(shape.n_pages), host_pages=40 * 36)
+    T = shape.frame_tokens
+    sid_of = {}
+    for it, ev in enumerate(steps):
+        for u in ev["suspend"]:
+            dp.suspend(sid_of[u])
+        for u in ev["resume"]:
+            dp.resume(sid_of[u])
+        for u in ev["open"]:
+            sid_of[u] = dp.open()
+        batch = [sid_of[u] for u in ev["batch"]]
+        cf = ev["chunk_frames"]
+        if batch:
+            n_tok = sum(cf) * T
+            q, k, v = (draw(rng, n_tok, shape) for _ in range(3))
+            if it % 5 == 0:
+                dp.attention(0, batch, cf, q, k, v, scale_of(shape))
+            dp.append(0, batch, cf, k, v)
+        for u in ev["close"]:
+            dp.close(sid_of.pop(u))
+        dp.check_state(list(sid_of.values()), kv=(it % 10 == 9))
+    assert max(len(e["batch"]) for e in steps) > 8
+
+
+# ---- configs[2] at full size, in the launch configuration bench.py times: sampled rows ----------------------
+def test_config2_full_size_sampled_rows():
+    w = synth.wan13b_batch()
+    shape = w.shape
+    T, H, D = shape.frame_tokens, shape.n_heads, shape.head_dim
+    dp = DualPool(shape, w.free_order)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(w.seed)
+    sids = [dp.open() for _ in w.sessions]
+    from synth.draw import draw_bits_torch
+    chunks = []
+    for sid, spec in zip(sids, w.sessions):
+        P = spec.prior_frames
+        for f in range(0, P, 3):
+            dk = draw_bits_torch(gen, 3 * T, H, D, "cuda")
+            dv = draw_bits_torch(gen, 3 * T, H, D, "cuda")
+            dp.append(0, [sid], [3], dev_to_bits(dk), dev_to_bits(dv), dev=(dk, dv))
+        chunks.append(tuple(draw_bits_torch(gen, 3 * T, H, D, "cuda") for _ in range(3)))
+    dp.check_state(sids, kv=False)
+    dq, dk, dv = (torch.cat([c[i] for c in chunks]) for i in range(3))
+    out = torch.full_like(dq, float("nan"))
+    lse = torch.empty(dq.shape[:2], dtype=torch.float32, device="cuda")
+    cf = [3] * len(sids)
+    dp.g.ts_chunk_attention(0, sids, cf, dq, dk, dv, out, lse, float(w.scale))
+    torch.cuda.synchronize()
+    o_gpu = out.double().cpu().numpy()
+    assert np.isfinite(o_gpu).all()
+    rs = np.random.default_rng(0)
+    C = 3 * T
+    errs, refs = [], []
+    for b, sid in enumerate(sids):
+        qb, kb, vb = (dev_to_bits(c) for c in chunks[b])
+        for _ in range(3):
+            h = int(rs.integers(0, H))
+            rows = np.unique(np.concatenate([rs.integers(0, C, size=24), [0, T - 1, T, 2 * T - 1, 2 * T, C - 1]]))
+            o_ref, l_ref = oracle.attention_rows(dp.o, 0, sid, 3, qb, kb, vb, w.scale, h, rows)
+            got = o_gpu[b * C + rows, h]
+            errs.append(got - o_ref)
+            refs.append(o_ref)
+            assert np.abs(lse[b * C + rows, h].double().cpu().numpy() - l_ref).max() <= 2e-3
+    err, ref = np.concatenate(errs), np.concatenate(refs)
+    assert np.abs(err).max() <= 2e-2
+    assert np.linalg.norm(err) / np.linalg.norm(ref) <= 5e-3
+    # property that holds at any size: appended bytes read back bit-exact for a sampled session
+    dp.append(0, sids, cf, dev_to_bits(dk), dev_to_bits(dv), dev=(dk, dv))
+    dp.check_state(sids[:2], kv=True)
