@@ -22,6 +22,11 @@ namespace tc {
 constexpr int kThreads = 384;
 constexpr int kTmemCols = 512;
 constexpr float kRescaleThresholdLog2 = 8.0f;   // lazy rescale: tolerate p up to 2^8 before touching O
+// Register file split (setmaxnreg): the CTA is launched with 384 x 168 registers; warps 0-3 (TMA, MMA, two idle)
+// drop to kRegsProducer so that the 8 softmax warps can hold a full 128-wide fp32 score row without spilling.
+constexpr int kRegsProducer = 72;
+constexpr int kRegsSoftmax = 216;
+static_assert(128 * kRegsProducer + 256 * kRegsSoftmax <= 384 * 168, "register pool");
 
 template <int D>
 struct Cfg {
@@ -115,6 +120,8 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
   const int it_begin = p.cta_begin[blockIdx.x];
   const int it_end = p.cta_begin[blockIdx.x + 1];
 
+  if (warp < 4) {
+    setmaxnreg_dec<kRegsProducer>();
   if (warp == 0) {
     // ===================================================================== TMA producer
     if (lane == 0) {
@@ -244,7 +251,9 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
         for (int i = 0; i < g.n_q; ++i) ++cnt_items[i];
       }
     }
-  } else if (warp >= 4) {
+  }
+  } else {
+    setmaxnreg_inc<kRegsSoftmax>();
     // ===================================================================== softmax + epilogue, one thread per query row
     const int wg = (warp - 4) >> 2;                       // query tile handled by this warpgroup
     const int row_in_tile = (warp & 3) * 32 + lane;
@@ -289,15 +298,17 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
           for (int k = 0; k < 128; ++k)
             if (k < lo || k >= hi) s[k] = 0xff800000u;   // -inf
         }
-        // ---- row max
+        // ---- row max (3-input FMNMX: two new values per instruction)
         float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]), mx3 = __uint_as_float(s[3]);
 #pragma unroll
-        for (int k = 4; k < 128; k += 4) {
-          mx0 = fmaxf(mx0, __uint_as_float(s[k]));
-          mx1 = fmaxf(mx1, __uint_as_float(s[k + 1]));
-          mx2 = fmaxf(mx2, __uint_as_float(s[k + 2]));
-          mx3 = fmaxf(mx3, __uint_as_float(s[k + 3]));
+        for (int k = 4; k < 124; k += 8) {
+          mx0 = max3(mx0, __uint_as_float(s[k + 0]), __uint_as_float(s[k + 1]));
+          mx1 = max3(mx1, __uint_as_float(s[k + 2]), __uint_as_float(s[k + 3]));
+          mx2 = max3(mx2, __uint_as_float(s[k + 4]), __uint_as_float(s[k + 5]));
+          mx3 = max3(mx3, __uint_as_float(s[k + 6]), __uint_as_float(s[k + 7]));
         }
+        mx0 = max3(mx0, __uint_as_float(s[124]), __uint_as_float(s[125]));
+        mx1 = max3(mx1, __uint_as_float(s[126]), __uint_as_float(s[127]));
         const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
         if (j == 0) {
           m = mx;   // the first tile of an item always holds a visible key for every row
@@ -317,28 +328,36 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
               tmem_ld32(taddr_o + cc, o);
               tmem_ld_wait();
 #pragma unroll
-              for (int k = 0; k < 32; ++k) o[k] = __float_as_uint(__uint_as_float(o[k]) * f);
+              for (int k = 0; k < 32; k += 2) {
+                float a0, a1;
+                mul2_bcast(a0, a1, __uint_as_float(o[k]), __uint_as_float(o[k + 1]), f);
+                o[k] = __float_as_uint(a0);
+                o[k + 1] = __float_as_uint(a1);
+              }
               tmem_st32(taddr_o + cc, o);
             }
           }
         }
         // ---- p = exp2(s*c - m*c); row sum; bf16 P back into TMEM (aliases the first 64 columns of S)
         const float neg_mc = -m * c;
-        float l0 = 0.f, l1 = 0.f;
+        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
 #pragma unroll
         for (int cc = 0; cc < 128; cc += 32) {
           uint32_t pk[16];
 #pragma unroll
-          for (int k = 0; k < 32; k += 2) {
-            const float p0 = ex2_approx(fmaf(__uint_as_float(s[cc + k]), c, neg_mc));
-            const float p1 = ex2_approx(fmaf(__uint_as_float(s[cc + k + 1]), c, neg_mc));
-            l0 += p0;
-            l1 += p1;
+          for (int k = 0; k < 32; k += 4) {
+            float x0, x1, x2, x3;
+            fma2_bcast(x0, x1, __uint_as_float(s[cc + k]), __uint_as_float(s[cc + k + 1]), c, neg_mc);
+            fma2_bcast(x2, x3, __uint_as_float(s[cc + k + 2]), __uint_as_float(s[cc + k + 3]), c, neg_mc);
+            const float p0 = ex2_approx(x0), p1 = ex2_approx(x1), p2 = ex2_approx(x2), p3 = ex2_approx(x3);
+            add2(l0, l1, p0, p1);
+            add2(l2, l3, p2, p3);
             pk[k >> 1] = pack_bf16x2(p0, p1);
+            pk[(k >> 1) + 1] = pack_bf16x2(p2, p3);
           }
           tmem_st16(taddr_s + (cc >> 1), pk);
         }
-        l += l0 + l1;
+        l += (l0 + l1) + (l2 + l3);
         tmem_st_wait();
         tc_fence_before();
         mbar_arrive(&p_full[wg]);

@@ -150,6 +150,56 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
 }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
+// ---------------------------------------------------------------- register reallocation between warpgroups
+template <int N>
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+
+// ---------------------------------------------------------------- packed fp32x2 math (sm_100 FFMA2 / FADD2: one issue slot per pair)
+// (d0, d1) = (a0, a1) * (b, b) + (c, c)
+__device__ __forceinline__ void fma2_bcast(float& d0, float& d1, float a0, float a1, float b, float c) {
+  asm("{\n"
+      ".reg .b64 ra, rb, rc;\n"
+      "mov.b64 ra, {%2, %3};\n"
+      "mov.b64 rb, {%4, %4};\n"
+      "mov.b64 rc, {%5, %5};\n"
+      "fma.rn.f32x2 ra, ra, rb, rc;\n"
+      "mov.b64 {%0, %1}, ra;\n"
+      "}\n"
+      : "=f"(d0), "=f"(d1)
+      : "f"(a0), "f"(a1), "f"(b), "f"(c));
+}
+// (d0, d1) += (a0, a1)
+__device__ __forceinline__ void add2(float& d0, float& d1, float a0, float a1) {
+  asm("{\n"
+      ".reg .b64 ra, rd;\n"
+      "mov.b64 rd, {%0, %1};\n"
+      "mov.b64 ra, {%2, %3};\n"
+      "add.f32x2 rd, rd, ra;\n"
+      "mov.b64 {%0, %1}, rd;\n"
+      "}\n"
+      : "+f"(d0), "+f"(d1)
+      : "f"(a0), "f"(a1));
+}
+// (d0, d1) = (a0, a1) * (b, b)
+__device__ __forceinline__ void mul2_bcast(float& d0, float& d1, float a0, float a1, float b) {
+  asm("{\n"
+      ".reg .b64 ra, rb;\n"
+      "mov.b64 ra, {%2, %3};\n"
+      "mov.b64 rb, {%4, %4};\n"
+      "mul.f32x2 ra, ra, rb;\n"
+      "mov.b64 {%0, %1}, ra;\n"
+      "}\n"
+      : "=f"(d0), "=f"(d1)
+      : "f"(a0), "f"(a1), "f"(b));
+}
+__device__ __forceinline__ float max3(float a, float b, float c) {
+  float d;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+  return d;
+}
+
 // ---------------------------------------------------------------- math
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
