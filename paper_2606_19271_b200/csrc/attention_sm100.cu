@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
     setmaxnreg_dec<kRegsProducer>();
   if (warp == 0) {
     // ===================================================================== TMA producer
-    if (lane == 0) {
+    if (elect_one()) {
       uint32_t kv_it = 0;
       uint32_t item_cnt = 0;
       for (int idx = it_begin; idx < it_end; ++idx, ++item_cnt) {
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
     }
   } else if (warp == 1) {
     // ===================================================================== MMA issuer
-    if (lane == 0) {
+    if (elect_one()) {
       constexpr uint32_t idesc_s = make_idesc_bf16(128, 128, 0, 0);
       constexpr uint32_t idesc_pv = make_idesc_bf16(128, D, 0, 1);
       const uint32_t sQ_addr = smem_u32(sQ);
