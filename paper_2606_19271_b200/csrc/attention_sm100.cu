@@ -9,16 +9,11 @@
 // Warp roles (384 threads):
 //   warp 0      TMA producer   Q tiles once per item, K/V tiles into a ring of kSlots smem slots
 //   warp 1      MMA issuer     tcgen05.mma, one elected thread; S = Q K^T (SS), O += P V (TS, P in TMEM)
-//   warps 4-7   softmax, key columns [0,64) of EVERY score tile   } two threads per query row: thread r of warp
-//   warps 8-11  softmax, key columns [64,128) of every score tile } 4+q and of warp 8+q own row 32q+r
-// Both softmax warpgroups work on the same score tile at the same time, so a tile's softmax takes half the
-// wall time of a one-thread-per-row split; that term sits on the S -> softmax -> PV -> S dependency chain of a
-// query tile, which is what bounds the kernel (the tensor pipe is fed by the OTHER query tile meanwhile).  The
-// two threads of a row exchange their partial row maximum (and, once per item, their partial row sum) through
-// shared memory and a 64-thread named barrier.  P is handed to the MMA warp in two halves (keys 0-31|64-95,
-// then 32-63|96-127) so that the first half of O += P V overlaps the second half of the exponentials.
+//   warps 4-7   softmax for query tile 0 (one thread per row): online softmax in fp32, lazy rescale of O,
+//   warps 8-11  softmax for query tile 1                        P written back to TMEM as bf16, epilogue
 // TMEM (512 columns): S0 [0,128) / P0 aliases [0,64); S1 [128,256) / P1; O0 [256,256+D); O1 [256+D,256+2D).
-// Issue order  S0(0) S1(0) | PV0(j) S0(j+1) PV1(j) S1(j+1) | ...  (two-tile ping-pong).
+// Issue order  S0(0) S1(0) | PV0(j) S0(j+1) PV1(j) S1(j+1) | ...  keeps the tensor pipe busy while the
+// other tile's softmax runs (two-tile ping-pong).
 #include "internal.h"
 #include "ptx.cuh"
 
@@ -28,40 +23,10 @@ constexpr int kThreads = 384;
 constexpr int kTmemCols = 512;
 constexpr float kRescaleThresholdLog2 = 8.0f;   // lazy rescale: tolerate p up to 2^8 before touching O
 // Register file split (setmaxnreg): the CTA is launched with 384 x 168 registers; warps 0-3 (TMA, MMA, two idle)
-// drop to kRegsProducer, the 8 softmax warps rise to kRegsSoftmax.
+// drop to kRegsProducer so that the 8 softmax warps can hold a full 128-wide fp32 score row without spilling.
 constexpr int kRegsProducer = 72;
 constexpr int kRegsSoftmax = 216;
 static_assert(128 * kRegsProducer + 256 * kRegsSoftmax <= 384 * 168, "register pool");
-
-// MUFU.EX2 runs at 16/clk/SM: one exp per (q,k) pair costs as many cycles as the pair's two MMAs at D=128, so a
-// share of the exponentials (kPolyPairs of every 16 element pairs) is evaluated on the FMA pipe instead.
-#ifndef TC_POLY_PAIRS
-#define TC_POLY_PAIRS 6
-#endif
-constexpr int kPolyPairs = TC_POLY_PAIRS;
-
-// 2^x for a packed pair on the FMA pipe (Cody-Waite): x = n + f with n = round(x), f in [-0.5, 0.5]; 2^f by a
-// degree-3 minimax polynomial (max relative error 7.5e-5, far below the 2^-9 of the bf16 rounding of P); 2^n by
-// adding n << 23 to the exponent field.  n sits in the low mantissa bits of x + 1.5*2^23.  x is clamped at -125
-// (masked scores are -inf), which yields 2^-125 instead of 0: negligible against a row sum >= 1.
-__device__ __forceinline__ void exp2_poly2(uint64_t x, float& p0, float& p1) {
-  float x0, x1;
-  upk2(x, x0, x1);
-  x0 = fmaxf(x0, -125.f);
-  x1 = fmaxf(x1, -125.f);
-  const uint64_t xc = pk2(x0, x1);
-  const uint64_t magic = pk2(12582912.f, 12582912.f);
-  const uint64_t xf = addp2(xc, magic);
-  const uint64_t fr = subp2(xc, subp2(xf, magic));
-  uint64_t p = fma2(pk2(0.05517083778977394f, 0.05517083778977394f), fr, pk2(0.24260935187339783f, 0.24260935187339783f));
-  p = fma2(p, fr, pk2(0.6932609677314758f, 0.6932609677314758f));
-  p = fma2(p, fr, pk2(0.9999281764030457f, 0.9999281764030457f));
-  float q0, q1, f0, f1;
-  upk2(p, q0, q1);
-  upk2(xf, f0, f1);
-  p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(f0) << 23));
-  p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(f1) << 23));
-}
 
 template <int D>
 struct Cfg {
@@ -72,8 +37,7 @@ struct Cfg {
   static constexpr int kSmemQ = 2 * kTileBytes;
   static constexpr int kSmemKV = kSlots * kTileBytes;
   static constexpr int kNumBars = 2 * kSlots + 2 + 10;
-  static constexpr int kXchgBytes = 2 * 2 * 128 * 4;    // [parity][column half][row] fp32 exchange slots
-  static constexpr int kSmemBytes = kSmemQ + kSmemKV + kXchgBytes + kNumBars * 8 + 16;
+  static constexpr int kSmemBytes = 1024 + kSmemQ + kSmemKV + kNumBars * 8 + 16;
 };
 
 struct ItemGeom {
@@ -112,26 +76,25 @@ __device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int idx) {
 template <int D>
 __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __grid_constant__ AttnParams p) {
   using C = Cfg<D>;
-  extern __shared__ __align__(1024) uint8_t smem[];   // swizzle-128B operands need 1024-byte alignment
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sQ = smem;
   uint8_t* sKV = smem + C::kSmemQ;
-  float* xchg = reinterpret_cast<float*>(sKV + C::kSmemKV);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + C::kSmemKV + C::kXchgBytes);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + C::kSmemKV);
   uint64_t* kv_full = bars;
   uint64_t* kv_empty = bars + C::kSlots;
   uint64_t* q_full = bars + 2 * C::kSlots;
   uint64_t* q_empty = q_full + 1;
-  uint64_t* s_full = q_full + 2;    // [2]   S tile i written by the tensor pipe
-  uint64_t* p_half = q_full + 4;    // [2][2] P tile i, half h (keys 32h..32h+31 and 64+32h..64+32h+31) written by softmax
-  uint64_t* o_done = q_full + 8;    // [2]   O tile i accumulated through the last issued PV
-  uint64_t* o_free = q_full + 10;   // [2]   O tile i read out by the epilogue
+  uint64_t* s_full = q_full + 2;    // [2]
+  uint64_t* p_half = q_full + 4;    // [2][2] P tile i, keys [64h, 64h+64) written by softmax
+  uint64_t* o_done = q_full + 8;    // [2]
+  uint64_t* o_free = q_full + 10;   // [2]
   uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + C::kNumBars);
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
-    if (smem_u32(smem) & 1023u) __trap();
     for (int i = 0; i < C::kSlots; ++i) {
       mbar_init(&kv_full[i], 1);
       mbar_init(&kv_empty[i], 1);
@@ -140,10 +103,10 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
     mbar_init(q_empty, 1);
     for (int i = 0; i < 2; ++i) {
       mbar_init(&s_full[i], 1);
-      mbar_init(&p_half[2 * i], 256);
-      mbar_init(&p_half[2 * i + 1], 256);
+      mbar_init(&p_half[2 * i], 128);
+      mbar_init(&p_half[2 * i + 1], 128);
       mbar_init(&o_done[i], 1);
-      mbar_init(&o_free[i], 256);
+      mbar_init(&o_free[i], 128);
     }
     fence_mbar_init();
     tma_prefetch_desc(&p.map_k);
@@ -228,12 +191,12 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
                  idesc_s, kk > 0);
         }
       };
-      // half h of O_i += P_i V: the 16-key steps {2h, 2h+1, 4+2h, 4+2h+1}, i.e. keys 32h.. and 64+32h..
+      // half h of O_i += P_i V: the 16-key steps 4h .. 4h+3 (keys [64h, 64h+64))
       auto issue_pv_half = [&](int i, uint32_t slot, int h, bool acc) {
         const uint32_t b = sKV_addr + slot * C::kTileBytes;
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-          const int kk = (q >> 1) * 4 + 2 * h + (q & 1);
+          const int kk = 4 * h + q;
           mma_ts(tmem_base + 256 + i * D, tmem_base + i * 128 + kk * 8,
                  make_smem_desc_sw128(b + kk * 2048, C::kBlockBytes, 1024), idesc_pv, (acc || q > 0) ? 1u : 0u);
         }
@@ -299,180 +262,144 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
   }
   } else {
     setmaxnreg_inc<kRegsSoftmax>();
-    // ===================================================================== softmax + epilogue, two threads per query row
-    const int half = (warp - 4) >> 2;                     // key columns [64*half, 64*half + 64) of every S tile
-    const int quarter = warp & 3;                         // TMEM lane quarter: rows [32*quarter, +32) of a query tile
-    const int row_in_tile = quarter * 32 + lane;
-    const uint32_t lane_sel = (uint32_t)(quarter * 32) << 16;
+    // ===================================================================== softmax + epilogue, one thread per query row
+    const int wg = (warp - 4) >> 2;                       // query tile handled by this warpgroup
+    const int row_in_tile = (warp & 3) * 32 + lane;
+    const uint32_t lane_sel = (uint32_t)((warp & 3) * 32) << 16;
+    const uint32_t taddr_s = tmem_base + lane_sel + wg * 128;
+    const uint32_t taddr_o = tmem_base + lane_sel + 256 + wg * D;
     const float c = p.scale_log2;
     const float thr = kRescaleThresholdLog2 / c;
-    uint32_t n_x = 0;                                     // exchange rounds so far (parity selects the slot set)
-    // swap a per-row value with the thread that owns the other column half of the same row
-    auto exchange = [&](float v) -> float {
-      float* slot = xchg + (n_x & 1) * 256;
-      ++n_x;
-      slot[half * 128 + row_in_tile] = v;
-      named_bar_sync(1 + quarter, 64);
-      return slot[(half ^ 1) * 128 + row_in_tile];
-    };
-    uint32_t cnt_s[2] = {0, 0}, cnt_pv[2] = {0, 0};
+    uint32_t cnt_s = 0, cnt_pv = 0;
     for (int idx = it_begin; idx < it_end; ++idx) {
       const ItemGeom g = decode_item(p, idx);
-      int lim_row[2], lim_min[2];
-      float m[2] = {-INFINITY, -INFINITY}, l[2] = {0.f, 0.f};
-#pragma unroll
-      for (int i = 0; i < 2; ++i) {
-        const int first_row = g.r0 + 128 * i;
-        const int row = first_row + row_in_tile;
-        lim_row[i] = min(g.C, (min(row, g.C - 1) / p.T + 1) * p.T);      // chunk keys visible to this row
-        lim_min[i] = min(g.C, (min(first_row, g.C - 1) / p.T + 1) * p.T);  // ... to the tile's first row
-      }
+      if (wg >= g.n_q) continue;
+      const int first_row = g.r0 + 128 * wg;
+      const int row = first_row + row_in_tile;
+      const int lim_row = min(g.C, (min(row, g.C - 1) / p.T + 1) * p.T);   // chunk keys visible to this row
+      const int lim_min = min(g.C, (first_row / p.T + 1) * p.T);           // ... to the tile's first row
+      float m = -INFINITY, l = 0.f;
       for (int j = 0; j < g.n_kv; ++j) {
+        mbar_wait(&s_full[wg], cnt_s & 1);
+        ++cnt_s;
+        tc_fence_after();
+        uint32_t s[128];
+        tmem_ld32(taddr_s + 0, s + 0);
+        tmem_ld32(taddr_s + 32, s + 32);
+        tmem_ld32(taddr_s + 64, s + 64);
+        tmem_ld32(taddr_s + 96, s + 96);
+        tmem_ld_wait();
+        // ---- mask (rare path)
+        int lo = 0, hi = 128;
+        bool need_mask;
+        if (j < g.n_prior) {
+          if (j == 0) lo = g.x_begin - (g.t0 << 7);
+          if (j == g.n_prior - 1) hi = g.x_end - ((g.t0 + j) << 7);
+          need_mask = (lo > 0) || (hi < 128);
+        } else {
+          const int base = (j - g.n_prior) << 7;
+          need_mask = base + 128 > lim_min;
+          hi = max(0, min(128, lim_row - base));
+        }
+        if (need_mask) {
 #pragma unroll
-        for (int i = 0; i < 2; ++i) {
-          if (i >= g.n_q) continue;
-          const uint32_t taddr_tile = tmem_base + lane_sel + i * 128;
-          mbar_wait(&s_full[i], cnt_s[i] & 1);
-          ++cnt_s[i];
-          tc_fence_after();
-          uint32_t s[64];
-          tmem_ld32(taddr_tile + half * 64, s);
-          tmem_ld32(taddr_tile + half * 64 + 32, s + 32);
-          tmem_ld_wait();
-          // ---- mask (rare path): own columns k stand for keys 64*half + k of the tile
-          int lo = 0, hi = 64;
-          bool need_mask;
-          if (j < g.n_prior) {
-            if (j == 0) lo = g.x_begin - (g.t0 << 7) - 64 * half;
-            if (j == g.n_prior - 1) hi = g.x_end - ((g.t0 + j) << 7) - 64 * half;
-            need_mask = (lo > 0) || (hi < 64);
-          } else {
-            const int base = (j - g.n_prior) << 7;
-            need_mask = base + 128 > lim_min[i];
-            hi = lim_row[i] - base - 64 * half;
-          }
-          if (need_mask) {
+          for (int k = 0; k < 128; ++k)
+            if (k < lo || k >= hi) s[k] = 0xff800000u;   // -inf
+        }
+        // ---- row max (3-input FMNMX: two new values per instruction)
+        float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]), mx3 = __uint_as_float(s[3]);
 #pragma unroll
-            for (int k = 0; k < 64; ++k)
-              if (k < lo || k >= hi) s[k] = 0xff800000u;   // -inf
-          }
-          // ---- row max over the own half (3-input FMNMX), then over the row through the partner thread
-          float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]), mx3 = __uint_as_float(s[3]);
+        for (int k = 4; k < 124; k += 8) {
+          mx0 = max3(mx0, __uint_as_float(s[k + 0]), __uint_as_float(s[k + 1]));
+          mx1 = max3(mx1, __uint_as_float(s[k + 2]), __uint_as_float(s[k + 3]));
+          mx2 = max3(mx2, __uint_as_float(s[k + 4]), __uint_as_float(s[k + 5]));
+          mx3 = max3(mx3, __uint_as_float(s[k + 6]), __uint_as_float(s[k + 7]));
+        }
+        mx0 = max3(mx0, __uint_as_float(s[124]), __uint_as_float(s[125]));
+        mx1 = max3(mx1, __uint_as_float(s[126]), __uint_as_float(s[127]));
+        const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+        if (j == 0) {
+          m = mx;   // the first tile of an item always holds a visible key for every row
+        } else {
+          const bool need = mx > m + thr;
+          if (__any_sync(0xffffffffu, need)) {
+            // rescale this warp's rows of O in TMEM: needs PV(j-1) of this tile complete
+            const float m_new = fmaxf(m, mx);
+            const float f = ex2_approx((m - m_new) * c);
+            l *= f;
+            m = m_new;
+            mbar_wait(&o_done[wg], (cnt_pv - 1) & 1);
+            tc_fence_after();
 #pragma unroll
-          for (int k = 4; k < 60; k += 8) {
-            mx0 = max3(mx0, __uint_as_float(s[k + 0]), __uint_as_float(s[k + 1]));
-            mx1 = max3(mx1, __uint_as_float(s[k + 2]), __uint_as_float(s[k + 3]));
-            mx2 = max3(mx2, __uint_as_float(s[k + 4]), __uint_as_float(s[k + 5]));
-            mx3 = max3(mx3, __uint_as_float(s[k + 6]), __uint_as_float(s[k + 7]));
-          }
-          mx0 = max3(mx0, __uint_as_float(s[60]), __uint_as_float(s[61]));
-          mx1 = max3(mx1, __uint_as_float(s[62]), __uint_as_float(s[63]));
-          const float mx_own = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-          const float mx = fmaxf(mx_own, exchange(mx_own));
-          if (j == 0) {
-            m[i] = mx;   // the first tile of an item always holds a visible key for every row
-          } else {
-            const bool need = mx > m[i] + thr;
-            if (__any_sync(0xffffffffu, need)) {
-              // rescale the own column half of this warp's rows of O in TMEM: needs PV(j-1) of this tile complete.
-              // The partner warp sees the same (mx, m) per row and takes the same branch.
-              const float m_new = fmaxf(m[i], mx);
-              const float f = ex2_approx((m[i] - m_new) * c);
-              l[i] *= f;
-              m[i] = m_new;
-              mbar_wait(&o_done[i], (cnt_pv[i] - 1) & 1);
-              tc_fence_after();
-              const uint32_t taddr_o = tmem_base + lane_sel + 256 + i * D + half * (D / 2);
+            for (int cc = 0; cc < D; cc += 32) {
+              uint32_t o[32];
+              tmem_ld32(taddr_o + cc, o);
+              tmem_ld_wait();
 #pragma unroll
-              for (int cc = 0; cc < D / 2; cc += 32) {
-                uint32_t o[32];
-                tmem_ld32(taddr_o + cc, o);
-                tmem_ld_wait();
-#pragma unroll
-                for (int k = 0; k < 32; k += 2) {
-                  float a0, a1;
-                  mul2_bcast(a0, a1, __uint_as_float(o[k]), __uint_as_float(o[k + 1]), f);
-                  o[k] = __float_as_uint(a0);
-                  o[k + 1] = __float_as_uint(a1);
-                }
-                tmem_st32(taddr_o + cc, o);
+              for (int k = 0; k < 32; k += 2) {
+                float a0, a1;
+                mul2_bcast(a0, a1, __uint_as_float(o[k]), __uint_as_float(o[k + 1]), f);
+                o[k] = __float_as_uint(a0);
+                o[k + 1] = __float_as_uint(a1);
               }
+              tmem_st32(taddr_o + cc, o);
             }
           }
-          // ---- p = exp2(s*c - m*c); row sum; bf16 P back into TMEM (P aliases the first 64 columns of S), in two
-          //      halves of 32 keys, each signalled to the MMA warp as soon as it is stored
-          const float neg_mc = -m[i] * c;
-          const uint64_t c2 = pk2(c, c), neg_mc2 = pk2(neg_mc, neg_mc);
-          uint64_t la = 0, lb = 0;   // packed (0.f, 0.f) row-sum accumulators
+        }
+        // ---- p = exp2(s*c - m*c); row sum; bf16 P back into TMEM (aliases the first 64 columns of S)
+        const float neg_mc = -m * c;
+        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
 #pragma unroll
-          for (int q2 = 0; q2 < 2; ++q2) {
-            uint32_t pk[16];
+        for (int cc = 0; cc < 128; cc += 32) {
+          uint32_t pk[16];
 #pragma unroll
-            for (int pi = 0; pi < 16; ++pi) {
-              const int k = 32 * q2 + 2 * pi;
-              const uint64_t x = fma2(pk2(__uint_as_float(s[k]), __uint_as_float(s[k + 1])), c2, neg_mc2);
-              float p0, p1;
-              // kPolyPairs of every 16 pairs take the FMA-pipe polynomial instead of MUFU.EX2 (spread evenly)
-              if (((pi + 1) * kPolyPairs) / 16 != (pi * kPolyPairs) / 16) {
-                exp2_poly2(x, p0, p1);
-              } else {
-                float x0, x1;
-                upk2(x, x0, x1);
-                p0 = ex2_approx(x0);
-                p1 = ex2_approx(x1);
-              }
-              if (pi & 1) lb = addp2(lb, pk2(p0, p1));
-              else la = addp2(la, pk2(p0, p1));
-              pk[pi] = pack_bf16x2(p0, p1);
-            }
-            tmem_st16(taddr_tile + 32 * half + 16 * q2, pk);
+          for (int k = 0; k < 32; k += 4) {
+            float x0, x1, x2, x3;
+            fma2_bcast(x0, x1, __uint_as_float(s[cc + k]), __uint_as_float(s[cc + k + 1]), c, neg_mc);
+            fma2_bcast(x2, x3, __uint_as_float(s[cc + k + 2]), __uint_as_float(s[cc + k + 3]), c, neg_mc);
+            const float p0 = ex2_approx(x0), p1 = ex2_approx(x1), p2 = ex2_approx(x2), p3 = ex2_approx(x3);
+            add2(l0, l1, p0, p1);
+            add2(l2, l3, p2, p3);
+            pk[k >> 1] = pack_bf16x2(p0, p1);
+            pk[(k >> 1) + 1] = pack_bf16x2(p2, p3);
+          }
+          tmem_st16(taddr_s + (cc >> 1), pk);
+          if (cc & 32) {   // a 64-key half of P is stored: hand it to the MMA warp
             tmem_st_wait();
             tc_fence_before();
-            mbar_arrive(&p_half[2 * i + q2]);
-          }
-          {
-            float l0, l1, l2, l3;
-            upk2(la, l0, l1);
-            upk2(lb, l2, l3);
-            l[i] += (l0 + l1) + (l2 + l3);
-          }
-          ++cnt_pv[i];
-        }
-      }
-      // ---- epilogue: O / l -> bf16 -> global (own column half of D), l summed over the two threads of the row
-#pragma unroll
-      for (int i = 0; i < 2; ++i) {
-        if (i >= g.n_q) continue;
-        const int row = g.r0 + 128 * i + row_in_tile;
-        const float l_row = l[i] + exchange(l[i]);
-        mbar_wait(&o_done[i], (cnt_pv[i] - 1) & 1);
-        tc_fence_after();
-        const float inv_l = 1.0f / l_row;
-        const bool store = row < g.C;
-        const uint32_t taddr_o = tmem_base + lane_sel + 256 + i * D + half * (D / 2);
-        uint16_t* orow = p.out + ((size_t)(g.q_off + row) * p.H + g.head) * D + half * (D / 2);
-#pragma unroll
-        for (int cc = 0; cc < D / 2; cc += 32) {
-          uint32_t o[32];
-          tmem_ld32(taddr_o + cc, o);
-          tmem_ld_wait();
-          if (store) {
-#pragma unroll
-            for (int k = 0; k < 32; k += 8) {
-              uint4 v;
-              v.x = pack_bf16x2(__uint_as_float(o[k + 0]) * inv_l, __uint_as_float(o[k + 1]) * inv_l);
-              v.y = pack_bf16x2(__uint_as_float(o[k + 2]) * inv_l, __uint_as_float(o[k + 3]) * inv_l);
-              v.z = pack_bf16x2(__uint_as_float(o[k + 4]) * inv_l, __uint_as_float(o[k + 5]) * inv_l);
-              v.w = pack_bf16x2(__uint_as_float(o[k + 6]) * inv_l, __uint_as_float(o[k + 7]) * inv_l);
-              *reinterpret_cast<uint4*>(orow + cc + k) = v;
-            }
+            mbar_arrive(&p_half[2 * wg + (cc >> 6)]);
           }
         }
-        tc_fence_before();
-        mbar_arrive(&o_free[i]);
-        if (p.lse != nullptr && store && half == 0)
-          p.lse[(size_t)(g.q_off + row) * p.H + g.head] = (m[i] * c + log2f(l_row)) * 0.6931471805599453f;
+        l += (l0 + l1) + (l2 + l3);
+        ++cnt_pv;
       }
+      // ---- epilogue: O / l -> bf16 -> global
+      mbar_wait(&o_done[wg], (cnt_pv - 1) & 1);
+      tc_fence_after();
+      const float inv_l = 1.0f / l;
+      const bool store = row < g.C;
+      uint16_t* orow = p.out + ((size_t)(g.q_off + row) * p.H + g.head) * D;
+#pragma unroll
+      for (int cc = 0; cc < D; cc += 32) {
+        uint32_t o[32];
+        tmem_ld32(taddr_o + cc, o);
+        tmem_ld_wait();
+        if (store) {
+#pragma unroll
+          for (int k = 0; k < 32; k += 8) {
+            uint4 v;
+            v.x = pack_bf16x2(__uint_as_float(o[k + 0]) * inv_l, __uint_as_float(o[k + 1]) * inv_l);
+            v.y = pack_bf16x2(__uint_as_float(o[k + 2]) * inv_l, __uint_as_float(o[k + 3]) * inv_l);
+            v.z = pack_bf16x2(__uint_as_float(o[k + 4]) * inv_l, __uint_as_float(o[k + 5]) * inv_l);
+            v.w = pack_bf16x2(__uint_as_float(o[k + 6]) * inv_l, __uint_as_float(o[k + 7]) * inv_l);
+            *reinterpret_cast<uint4*>(orow + cc + k) = v;
+          }
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(&o_free[wg]);
+      if (p.lse != nullptr && store)
+        p.lse[(size_t)(g.q_off + row) * p.H + g.head] = (m * c + log2f(l)) * 0.6931471805599453f;
     }
   }
 

@@ -527,15 +527,28 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
     for (int qp = 0; qp < n_pairs; ++qp) {
       int n_q, n_kv;
       item_geometry(c, C, d.x_begin, d.x_end, qp, &n_q, &n_kv);
-      const int cost = n_q * (n_kv + 2);      // +2: pipeline fill and epilogue, in KV-tile units
+      // time model in tenths of a two-tile KV step; +2: pipeline fill and epilogue.  A lone query tile has no
+      // ping-pong partner to hide its S -> softmax -> PV chain behind, so it runs at ~0.9 of a pair's step time.
+      const int cost = (n_q == 2 ? 20 : 18) * (n_kv + 2);
       for (int h = 0; h < H; ++h) cands.push_back({cost, b, h, qp, n_kv});
     }
     q_off += C;
     pt_off += (int)s.pt.size();
   }
-  // LPT: heaviest first, each to the least-loaded CTA.  Ties keep (session, head) neighbours adjacent so that
-  // CTAs running concurrently stream the same K/V pages through L2.
-  std::stable_sort(cands.begin(), cands.end(), [](const Cand& x, const Cand& y) { return x.cost > y.cost; });
+  // List scheduling in (session, head) stream order: the q-pair items of one stream read the same K/V pages, so they
+  // are dealt out back to back (each to the least-loaded CTA) and run at the same time on neighbouring CTAs - the
+  // stream's K/V then comes from DRAM once and from L2 for the other items.  Heaviest streams first (LPT at stream
+  // granularity) so that the tail of the schedule is made of short items.
+  {
+    std::vector<int64_t> stream_cost((size_t)n * H, 0);
+    for (const Cand& x : cands) stream_cost[(size_t)x.sess * H + x.head] += x.cost;
+    std::stable_sort(cands.begin(), cands.end(), [&](const Cand& x, const Cand& y) {
+      const size_t sx = (size_t)x.sess * H + x.head, sy = (size_t)y.sess * H + y.head;
+      if (stream_cost[sx] != stream_cost[sy]) return stream_cost[sx] > stream_cost[sy];
+      if (sx != sy) return sx < sy;
+      return x.cost > y.cost;
+    });
+  }
   std::vector<std::vector<int>> per_cta(grid);
   {
     typedef std::pair<int64_t, int> Load;   // (load, cta)
