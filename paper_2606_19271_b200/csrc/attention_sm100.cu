@@ -43,6 +43,8 @@ struct Cfg {
 struct ItemGeom {
   int sess, head, r0, n_q, C, q_off, pt_off, n_pt;
   int x_begin, x_end, t0, n_prior, n_chunk, n_kv;
+  int n_pipe;   // KV tiles flowing through the smem ring for this item (>= n_kv: the cluster partner may see more)
+  bool mc;      // K/V tiles are loaded half by this CTA, half by the cluster partner, multicast to both
 };
 
 __device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int idx) {
@@ -58,10 +60,8 @@ __device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int idx) {
   g.n_pt = s.n_pt;
   g.x_begin = s.x_begin;
   g.x_end = s.x_end;
-  g.n_q = (g.r0 + 128 < s.C) ? 2 : 1;
-  const int last_row = min(s.C, g.r0 + 256) - 1;
-  const int kv_hi = min(s.C, (last_row / p.T + 1) * p.T);   // chunk keys visible to the item's last row
-  g.n_chunk = (kv_hi + 127) >> 7;
+  g.n_pipe = (int)(w.pipe & 0xffffffu);
+  g.mc = (w.pipe >> 31) != 0;
   if (s.x_end > s.x_begin) {
     g.t0 = s.x_begin >> 7;
     g.n_prior = ((s.x_end - 1) >> 7) - g.t0 + 1;
@@ -69,7 +69,18 @@ __device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int idx) {
     g.t0 = 0;
     g.n_prior = 0;
   }
-  g.n_kv = g.n_prior + g.n_chunk;
+  if (w.q_pair < 0) {   // no query rows: only the loader and the slot releases run
+    g.r0 = 0;
+    g.n_q = 0;
+    g.n_chunk = 0;
+    g.n_kv = 0;
+  } else {
+    g.n_q = (g.r0 + 128 < s.C) ? 2 : 1;
+    const int last_row = min(s.C, g.r0 + 256) - 1;
+    const int kv_hi = min(s.C, (last_row / p.T + 1) * p.T);   // chunk keys visible to the item's last row
+    g.n_chunk = (kv_hi + 127) >> 7;
+    g.n_kv = g.n_prior + g.n_chunk;
+  }
   return g;
 }
 
@@ -97,7 +108,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
   if (warp == 0 && lane == 0) {
     for (int i = 0; i < C::kSlots; ++i) {
       mbar_init(&kv_full[i], 1);
-      mbar_init(&kv_empty[i], 1);
+      mbar_init(&kv_empty[i], 2);   // released by the MMA warps of both CTAs of the cluster
     }
     mbar_init(q_full, 1);
     mbar_init(q_empty, 1);
@@ -115,7 +126,9 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
   if (warp == 1) tmem_alloc(tmem_ptr, kTmemCols);
   tc_fence_before();
   __syncthreads();
+  cluster_sync_all();   // the partner's barriers are initialised before any multicast load or commit reaches them
   tc_fence_after();
+  const uint32_t cta_rank = cluster_ctarank();
   const uint32_t tmem_base = *tmem_ptr;
 
   const int it_begin = p.cta_begin[blockIdx.x];
@@ -127,48 +140,56 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
     // ===================================================================== TMA producer
     if (elect_one()) {
       uint32_t kv_it = 0;
-      uint32_t item_cnt = 0;
-      for (int idx = it_begin; idx < it_end; ++idx, ++item_cnt) {
+      uint32_t q_cnt = 0;
+      const int sb = min(p.B, 64);            // tokens per TMA box of K/V (the maps are encoded with this box)
+      const int n_sub = 128 / sb;             // boxes per 128-key tile
+      for (int idx = it_begin; idx < it_end; ++idx) {
         const ItemGeom g = decode_item(p, idx);
         const CUtensorMap* mq = p.sess_maps + g.sess * 3;
         const CUtensorMap* mkn = mq + 1;
         const CUtensorMap* mvn = mq + 2;
         const int32_t* pt = p.page_tables + g.pt_off;
-        mbar_wait(q_empty, (item_cnt & 1) ^ 1);
-        mbar_arrive_expect_tx(q_full, g.n_q * C::kTileBytes);
-        for (int i = 0; i < g.n_q; ++i)
-          for (int b = 0; b < C::kDBlocks; ++b)
-            tma_load_3d(sQ + i * C::kTileBytes + b * C::kBlockBytes, mq, 64 * b, g.head, g.r0 + 128 * i, q_full);
-        for (int j = 0; j < g.n_kv; ++j) {
+        if (g.n_q > 0) {
+          mbar_wait_long(q_empty, (q_cnt & 1) ^ 1);
+          ++q_cnt;
+          mbar_arrive_expect_tx(q_full, g.n_q * C::kTileBytes);
+          for (int i = 0; i < g.n_q; ++i)
+            for (int b = 0; b < C::kDBlocks; ++b)
+              tma_load_3d(sQ + i * C::kTileBytes + b * C::kBlockBytes, mq, 64 * b, g.head, g.r0 + 128 * i, q_full);
+        }
+        for (int j = 0; j < g.n_pipe; ++j) {
           for (int kv = 0; kv < 2; ++kv, ++kv_it) {
             const uint32_t slot = kv_it % C::kSlots;
             const uint32_t ph = (kv_it / C::kSlots) & 1;
-            mbar_wait(&kv_empty[slot], ph ^ 1);
-            mbar_arrive_expect_tx(&kv_full[slot], C::kTileBytes);
+            mbar_wait_long(&kv_empty[slot], ph ^ 1);
+            if (!g.mc && j >= g.n_kv) {
+              // a tile of the partner's unrelated item: nothing to load, but the slot is cycled so that both CTAs
+              // of the cluster stay on the same ring position (multicast needs equal smem offsets)
+              mbar_arrive(&kv_full[slot]);
+              continue;
+            }
+            mbar_arrive_expect_tx(&kv_full[slot], C::kTileBytes);   // own boxes + (multicast) the partner's
             uint8_t* dst = sKV + slot * C::kTileBytes;
-            if (j < g.n_prior) {
-              const CUtensorMap* mc = kv ? &p.map_v : &p.map_k;
-              const int t = g.t0 + j;
-              if (p.B >= 128) {
-                const int x = t << 7;
-                const int page = pt[x >> p.log2_B];
-                const int tok0 = x & (p.B - 1);
-                for (int b = 0; b < C::kDBlocks; ++b)
-                  tma_load_4d(dst + b * C::kBlockBytes, mc, 64 * b, tok0, g.head, page, &kv_full[slot]);
+            for (int sx = 0; sx < n_sub; ++sx) {
+              if (g.mc && (uint32_t)(sx & 1) != cta_rank) continue;   // the partner loads and multicasts this box
+              uint8_t* d = dst + sx * sb * 128;
+              if (j < g.n_prior) {
+                const CUtensorMap* mc = kv ? &p.map_v : &p.map_k;
+                const int x = ((g.t0 + j) << 7) + sx * sb;            // page-table coordinate of the box
+                const int page = pt[min(x >> p.log2_B, g.n_pt - 1)];  // past-the-end boxes re-read the last page (masked)
+                const int tok = x & (p.B - 1);
+                for (int b = 0; b < C::kDBlocks; ++b) {
+                  if (g.mc) tma_load_4d_mc(d + b * C::kBlockBytes, mc, 64 * b, tok, g.head, page, &kv_full[slot], 3);
+                  else tma_load_4d(d + b * C::kBlockBytes, mc, 64 * b, tok, g.head, page, &kv_full[slot]);
+                }
               } else {
-                const int per = 128 >> p.log2_B;      // pages per 128-key tile
-                for (int s = 0; s < per; ++s) {
-                  const int pidx = min(t * per + s, g.n_pt - 1);   // past-the-end sub-tiles re-read the last page (masked)
-                  const int page = pt[pidx];
-                  for (int b = 0; b < C::kDBlocks; ++b)
-                    tma_load_4d(dst + b * C::kBlockBytes + s * p.B * 128, mc, 64 * b, 0, g.head, page, &kv_full[slot]);
+                const CUtensorMap* mc = kv ? mvn : mkn;
+                const int row = ((j - g.n_prior) << 7) + sx * sb;
+                for (int b = 0; b < C::kDBlocks; ++b) {
+                  if (g.mc) tma_load_3d_mc(d + b * C::kBlockBytes, mc, 64 * b, g.head, row, &kv_full[slot], 3);
+                  else tma_load_3d(d + b * C::kBlockBytes, mc, 64 * b, g.head, row, &kv_full[slot]);
                 }
               }
-            } else {
-              const int u = j - g.n_prior;
-              const CUtensorMap* mc = kv ? mvn : mkn;
-              for (int b = 0; b < C::kDBlocks; ++b)
-                tma_load_3d(dst + b * C::kBlockBytes, mc, 64 * b, g.head, 128 * u, &kv_full[slot]);
             }
           }
         }
@@ -201,13 +222,18 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
                  make_smem_desc_sw128(b + kk * 2048, C::kBlockBytes, 1024), idesc_pv, (acc || q > 0) ? 1u : 0u);
         }
       };
-      uint32_t kv_it = 0, item_cnt = 0;
+      uint32_t kv_it = 0, q_cnt = 0;
       uint32_t cnt_p[2] = {0, 0};
       uint32_t cnt_items[2] = {0, 0};
-      for (int idx = it_begin; idx < it_end; ++idx, ++item_cnt) {
+      for (int idx = it_begin; idx < it_end; ++idx) {
         const ItemGeom g = decode_item(p, idx);
-        mbar_wait(q_full, item_cnt & 1);
-        {
+        // hand a K/V slot back once every MMA issued so far has read it - always to BOTH CTAs of the cluster, also
+        // when the two work on unrelated items: a slot is refilled (possibly by the partner's multicast) only after
+        // both CTAs are done with their tile at that ring position
+        auto release = [&](uint32_t slot) { mma_commit_mc(&kv_empty[slot], 3); };
+        if (g.n_q > 0) {
+          mbar_wait(q_full, q_cnt & 1);
+          ++q_cnt;
           const uint32_t slot = kv_it % C::kSlots, ph = (kv_it / C::kSlots) & 1;
           ++kv_it;
           mbar_wait(&kv_full[slot], ph);
@@ -216,7 +242,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
             issue_s(i, slot);
             mma_commit(&s_full[i]);
           }
-          mma_commit(&kv_empty[slot]);
+          release(slot);
           if (g.n_kv == 1) mma_commit(q_empty);
         }
         for (int j = 0; j < g.n_kv; ++j) {
@@ -241,7 +267,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
             tc_fence_after();
             issue_pv_half(i, slot_v, 1, true);
             mma_commit(&o_done[i]);
-            if (i == g.n_q - 1) mma_commit(&kv_empty[slot_v]);
+            if (i == g.n_q - 1) release(slot_v);
             if (has_next) {
               if (i == 0) {
                 mbar_wait(&kv_full[slot_k], ph_k);
@@ -250,13 +276,20 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
               issue_s(i, slot_k);
               mma_commit(&s_full[i]);
               if (i == g.n_q - 1) {
-                mma_commit(&kv_empty[slot_k]);
+                release(slot_k);
                 if (j + 2 == g.n_kv) mma_commit(q_empty);
               }
             }
           }
         }
         for (int i = 0; i < g.n_q; ++i) ++cnt_items[i];
+        // K/V tiles only the cluster partner needs (it sees more chunk frames, or this CTA has no query rows)
+        for (int e = 2 * g.n_kv; e < 2 * g.n_pipe; ++e) {
+          const uint32_t slot = kv_it % C::kSlots, ph = (kv_it / C::kSlots) & 1;
+          ++kv_it;
+          mbar_wait(&kv_full[slot], ph);
+          release(slot);
+        }
       }
     }
   }
@@ -405,31 +438,40 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
 
   tc_fence_before();
   __syncthreads();
+  cluster_sync_all();   // no CTA exits while its partner may still multicast into it or arrive on its barriers
   if (warp == 1) tmem_dealloc(tmem_base, kTmemCols);
 }
 
 int attention_smem_bytes(int head_dim) { return head_dim == 128 ? Cfg<128>::kSmemBytes : Cfg<64>::kSmemBytes; }
 
-cudaError_t launch_attention(const AttnParams& p, int head_dim, int grid, cudaStream_t stream) {
-  static bool configured[2] = {false, false};
-  if (head_dim == 128) {
-    if (!configured[0]) {
-      cudaError_t e = cudaFuncSetAttribute(chunk_attention_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           Cfg<128>::kSmemBytes);
-      if (e != cudaSuccess) return e;
-      configured[0] = true;
-    }
-    chunk_attention_kernel<128><<<grid, kThreads, Cfg<128>::kSmemBytes, stream>>>(p);
-  } else {
-    if (!configured[1]) {
-      cudaError_t e = cudaFuncSetAttribute(chunk_attention_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           Cfg<64>::kSmemBytes);
-      if (e != cudaSuccess) return e;
-      configured[1] = true;
-    }
-    chunk_attention_kernel<64><<<grid, kThreads, Cfg<64>::kSmemBytes, stream>>>(p);
+template <int D>
+static cudaError_t launch_clustered(const AttnParams& p, int grid, cudaStream_t stream) {
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(chunk_attention_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         Cfg<D>::kSmemBytes);
+    if (e != cudaSuccess) return e;
+    configured = true;
   }
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid, 1, 1);
+  cfg.blockDim = dim3(kThreads, 1, 1);
+  cfg.dynamicSmemBytes = Cfg<D>::kSmemBytes;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2;   // CTA pairs: K/V tiles of a shared (session, head) are loaded once per pair
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, chunk_attention_kernel<D>, p);
+}
+
+// grid must be even: CTAs 2c and 2c+1 form cluster c and walk item lists of equal length.
+cudaError_t launch_attention(const AttnParams& p, int head_dim, int grid, cudaStream_t stream) {
+  if (grid <= 0 || (grid & 1)) return cudaErrorInvalidValue;
+  return head_dim == 128 ? launch_clustered<128>(p, grid, stream) : launch_clustered<64>(p, grid, stream);
 }
 
 }  // namespace tc

@@ -365,7 +365,7 @@ int ts_pool_create(const ts_pool_config* cfg, ts_pool** out) {
                               (cuuint64_t)cfg->n_pages};
   const cuuint64_t strides[3] = {(cuuint64_t)cfg->head_dim * 2, (cuuint64_t)cfg->page_tokens * cfg->head_dim * 2,
                                  (cuuint64_t)page_bytes};
-  const cuuint32_t box[4] = {64, (cuuint32_t)std::min(cfg->page_tokens, 128), 1, 1};
+  const cuuint32_t box[4] = {64, (cuuint32_t)std::min(cfg->page_tokens, 64), 1, 1};   // half a 128-key tile at most
   for (int l = 0; l < cfg->n_layers; ++l) {
     uint8_t* base = pool->slab + (int64_t)l * pool->layer_bytes;
     if (!encode_map(&pool->map_k[l], base, 4, dims, strides, box)) return fail(TS_ERR_CUDA);
@@ -476,15 +476,17 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
     n_pt_total += pool->sess[sids[b]].pt.size();
     n_items += H * ((chunk_frames[b] * T + 255) / 256);
   }
-  const int grid = std::min(pool->sm_count, n_items);
+  // items are dealt to CTA pairs (2-CTA clusters): at most one cluster item per candidate, two CTA entries each
+  n_items *= 2;
+  const int grid_max = std::max(2, pool->sm_count & ~1);
   ScheduleLayout L;
   L.n_items = n_items;
-  L.grid = grid;
+  L.grid = grid_max;
   L.off_maps = 0;
   L.off_sess = align_up(L.off_maps + (size_t)n * 3 * sizeof(CUtensorMap), 128);
   L.off_pt = align_up(L.off_sess + (size_t)n * sizeof(SessDesc), 128);
   L.off_cta = align_up(L.off_pt + n_pt_total * 4, 128);
-  L.off_items = align_up(L.off_cta + (size_t)(grid + 1) * 4, 128);
+  L.off_items = align_up(L.off_cta + (size_t)(grid_max + 1) * 4, 128);
   L.bytes = L.off_items + (size_t)n_items * sizeof(WorkItem);
   Staging* st = nullptr;
   rc = acquire_staging(pool, L.bytes, &st);
@@ -518,11 +520,12 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
     // per-session 3D maps {D, H, C}: rows past the session's chunk read as zeros, never as a neighbour's tokens
     const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)H, (cuuint64_t)C};
     const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)H * D * 2};
-    const cuuint32_t box[3] = {64, 1, 128};
+    const cuuint32_t box_q[3] = {64, 1, 128};
+    const cuuint32_t box_kv[3] = {64, 1, (cuuint32_t)std::min(c.page_tokens, 64)};   // same box rows as the cache maps
     const size_t byte_off = (size_t)q_off * H * D * 2;
-    if (!encode_map(&maps[b * 3 + 0], (uint8_t*)q + byte_off, 3, dims, strides, box)) return TS_ERR_CUDA;
-    if (!encode_map(&maps[b * 3 + 1], (uint8_t*)k + byte_off, 3, dims, strides, box)) return TS_ERR_CUDA;
-    if (!encode_map(&maps[b * 3 + 2], (uint8_t*)v + byte_off, 3, dims, strides, box)) return TS_ERR_CUDA;
+    if (!encode_map(&maps[b * 3 + 0], (uint8_t*)q + byte_off, 3, dims, strides, box_q)) return TS_ERR_CUDA;
+    if (!encode_map(&maps[b * 3 + 1], (uint8_t*)k + byte_off, 3, dims, strides, box_kv)) return TS_ERR_CUDA;
+    if (!encode_map(&maps[b * 3 + 2], (uint8_t*)v + byte_off, 3, dims, strides, box_kv)) return TS_ERR_CUDA;
     const int n_pairs = (C + 255) / 256;
     for (int qp = 0; qp < n_pairs; ++qp) {
       int n_q, n_kv;
@@ -535,40 +538,77 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
     q_off += C;
     pt_off += (int)s.pt.size();
   }
-  // List scheduling in (session, head) stream order: the q-pair items of one stream read the same K/V pages, so they
-  // are dealt out back to back (each to the least-loaded CTA) and run at the same time on neighbouring CTAs - the
-  // stream's K/V then comes from DRAM once and from L2 for the other items.  Heaviest streams first (LPT at stream
-  // granularity) so that the tail of the schedule is made of short items.
-  {
-    std::vector<int64_t> stream_cost((size_t)n * H, 0);
-    for (const Cand& x : cands) stream_cost[(size_t)x.sess * H + x.head] += x.cost;
-    std::stable_sort(cands.begin(), cands.end(), [&](const Cand& x, const Cand& y) {
-      const size_t sx = (size_t)x.sess * H + x.head, sy = (size_t)y.sess * H + y.head;
-      if (stream_cost[sx] != stream_cost[sy]) return stream_cost[sx] > stream_cost[sy];
-      if (sx != sy) return sx < sy;
-      return x.cost > y.cost;
-    });
+  // ---- cluster items.  The q-pair items of one (session, head) stream read the same K/V pages: two of them at a
+  // time go to the two CTAs of a cluster, which then load half of every K/V tile each and multicast it to both
+  // (mc).  A stream's odd item out is paired with another stream's (or with nothing): those two share a cluster
+  // without sharing loads.  Both CTAs cycle max(n_kv) tiles through their smem rings so that they stay on the same
+  // ring position.
+  struct CItem {
+    int cost;
+    int64_t stream_cost;
+    int stream;
+    Cand a, b;       // b.q_pair < 0: no second item
+    bool mc;
+  };
+  std::vector<int64_t> stream_cost((size_t)n * H, 0);
+  for (const Cand& x : cands) stream_cost[(size_t)x.sess * H + x.head] += x.cost;
+  std::stable_sort(cands.begin(), cands.end(), [&](const Cand& x, const Cand& y) {
+    const size_t sx = (size_t)x.sess * H + x.head, sy = (size_t)y.sess * H + y.head;
+    if (sx != sy) return sx < sy;
+    return x.cost > y.cost;
+  });
+  std::vector<CItem> citems;
+  std::vector<Cand> odd;
+  for (size_t i = 0; i < cands.size();) {
+    size_t e = i;
+    while (e < cands.size() && cands[e].sess == cands[i].sess && cands[e].head == cands[i].head) ++e;
+    const int stream = cands[i].sess * H + cands[i].head;
+    for (; i + 1 < e; i += 2)
+      citems.push_back({std::max(cands[i].cost, cands[i + 1].cost), stream_cost[stream], stream, cands[i], cands[i + 1], true});
+    if (i < e) odd.push_back(cands[i++]);
   }
-  std::vector<std::vector<int>> per_cta(grid);
+  std::stable_sort(odd.begin(), odd.end(), [](const Cand& x, const Cand& y) { return x.cost > y.cost; });
+  for (size_t i = 0; i < odd.size(); i += 2) {
+    Cand none = odd[i];
+    none.q_pair = -1;
+    none.n_kv = 0;
+    none.cost = 0;
+    const Cand& second = (i + 1 < odd.size()) ? odd[i + 1] : none;
+    const int stream = odd[i].sess * H + odd[i].head;
+    citems.push_back({std::max(odd[i].cost, second.cost), stream_cost[stream], stream, odd[i], second, false});
+  }
+  // List scheduling in stream order, heaviest streams first (LPT at stream granularity, so that the tail of the
+  // schedule is made of short items): a stream's items are dealt out back to back, each to the least-loaded
+  // cluster, and run at the same time - the stream's K/V then comes from DRAM once and from L2 afterwards.
+  std::stable_sort(citems.begin(), citems.end(), [](const CItem& x, const CItem& y) {
+    if (x.stream_cost != y.stream_cost) return x.stream_cost > y.stream_cost;
+    if (x.stream != y.stream) return x.stream < y.stream;
+    return x.cost > y.cost;
+  });
+  const int n_clusters = std::min(grid_max / 2, (int)citems.size());
+  const int grid = 2 * n_clusters;
+  std::vector<std::vector<int>> per_cluster(n_clusters);
   {
-    typedef std::pair<int64_t, int> Load;   // (load, cta)
+    typedef std::pair<int64_t, int> Load;   // (load, cluster)
     std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
-    for (int i = 0; i < grid; ++i) heap.push({0, i});
-    for (int i = 0; i < (int)cands.size(); ++i) {
+    for (int i = 0; i < n_clusters; ++i) heap.push({0, i});
+    for (int i = 0; i < (int)citems.size(); ++i) {
       Load top = heap.top();
       heap.pop();
-      per_cta[top.second].push_back(i);
-      heap.push({top.first + cands[i].cost, top.second});
+      per_cluster[top.second].push_back(i);
+      heap.push({top.first + citems[i].cost, top.second});
     }
   }
   int w = 0;
   for (int ci = 0; ci < grid; ++ci) {
     cta_begin[ci] = w;
-    for (int i : per_cta[ci]) {
-      items[w].sess = cands[i].sess;
-      items[w].head = cands[i].head;
-      items[w].q_pair = cands[i].q_pair;
-      items[w].n_kv = cands[i].n_kv;
+    for (int i : per_cluster[ci >> 1]) {
+      const CItem& it = citems[i];
+      const Cand& x = (ci & 1) ? it.b : it.a;
+      items[w].sess = x.sess;
+      items[w].head = x.head;
+      items[w].q_pair = x.q_pair;
+      items[w].pipe = (uint32_t)std::max(it.a.n_kv, it.b.n_kv) | (it.mc ? 0x80000000u : 0u);
       ++w;
     }
   }
