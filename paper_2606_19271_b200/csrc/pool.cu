@@ -530,9 +530,10 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
     for (int qp = 0; qp < n_pairs; ++qp) {
       int n_q, n_kv;
       item_geometry(c, C, d.x_begin, d.x_end, qp, &n_q, &n_kv);
-      // time model in tenths of a two-tile KV step; +2: pipeline fill and epilogue.  A lone query tile has no
-      // ping-pong partner to hide its S -> softmax -> PV chain behind, so it runs at ~0.9 of a pair's step time.
-      const int cost = (n_q == 2 ? 20 : 18) * (n_kv + 2);
+      // time model in twentieths of a two-tile KV step, fitted to per-CTA cycle counts on configs[2]
+      // (3184 clk per step + 14.7 k clk per item): 4.5 steps per item for the Q load, pipeline fill and epilogue.
+      // A lone query tile has no ping-pong partner to hide its S -> softmax -> PV chain behind: ~0.95 of a pair step.
+      const int cost = (n_q == 2 ? 20 : 19) * n_kv + 90;
       for (int h = 0; h < H; ++h) cands.push_back({cost, b, h, qp, n_kv});
     }
     q_off += C;
@@ -552,9 +553,11 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   };
   std::vector<int64_t> stream_cost((size_t)n * H, 0);
   for (const Cand& x : cands) stream_cost[(size_t)x.sess * H + x.head] += x.cost;
+  // within a stream: by KV length (longest first), two-tile items before a lone tile
   std::stable_sort(cands.begin(), cands.end(), [&](const Cand& x, const Cand& y) {
     const size_t sx = (size_t)x.sess * H + x.head, sy = (size_t)y.sess * H + y.head;
     if (sx != sy) return sx < sy;
+    if (x.n_kv != y.n_kv) return x.n_kv > y.n_kv;
     return x.cost > y.cost;
   });
   std::vector<CItem> citems;
@@ -563,9 +566,21 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
     size_t e = i;
     while (e < cands.size() && cands[e].sess == cands[i].sess && cands[e].head == cands[i].head) ++e;
     const int stream = cands[i].sess * H + cands[i].head;
-    for (; i + 1 < e; i += 2)
-      citems.push_back({std::max(cands[i].cost, cands[i + 1].cost), stream_cost[stream], stream, cands[i], cands[i + 1], true});
-    if (i < e) odd.push_back(cands[i++]);
+    // pair items of EQUAL KV length first (neither CTA then waits for tiles only its partner needs); what is left
+    // over (at most one item per length) is paired in length order, and the stream's last odd item goes to `odd`
+    std::vector<Cand> rest;
+    while (i < e) {
+      if (i + 1 < e && cands[i].n_kv == cands[i + 1].n_kv) {
+        citems.push_back({std::max(cands[i].cost, cands[i + 1].cost), stream_cost[stream], stream, cands[i], cands[i + 1], true});
+        i += 2;
+      } else {
+        rest.push_back(cands[i++]);
+      }
+    }
+    size_t r = 0;
+    for (; r + 1 < rest.size(); r += 2)
+      citems.push_back({std::max(rest[r].cost, rest[r + 1].cost), stream_cost[stream], stream, rest[r], rest[r + 1], true});
+    if (r < rest.size()) odd.push_back(rest[r]);
   }
   std::stable_sort(odd.begin(), odd.end(), [](const Cand& x, const Cand& y) { return x.cost > y.cost; });
   for (size_t i = 0; i < odd.size(); i += 2) {
