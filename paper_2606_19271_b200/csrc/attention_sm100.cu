@@ -1,10 +1,10 @@
 // Coalesced chunk attention for sm_100a (step a2 of SURVEY.md §8(a); PAPER.md:66 (iii)).
 //
-// One persistent CTA per SM walks a host-balanced list of work items (session, head, pair of 128-row
-// query tiles).  Per item the KV sequence is: the session's visible cached tokens in PHYSICAL page order
-// (softmax is order-invariant over keys), gathered page by page through the page table with TMA, then the
-// chunk's own K/V tiles from the packed call tensors.  Only the first/last cache tile and the chunk tiles
-// that cross a frame boundary take the masked path.
+// Persistent CTAs, one per SM, in 2-CTA clusters.  Each CTA walks a host-built list of work items (session, head,
+// pair of 128-row query tiles).  Per item the KV sequence is: the session's visible cached tokens in PHYSICAL page
+// order (softmax is order-invariant over keys), gathered page by page through the page table with TMA, then the
+// chunk's own K/V tiles from the packed call tensors.  Only the first/last cache tile and the chunk tiles that
+// cross a frame boundary take the masked path.
 //
 // Warp roles (384 threads):
 //   warp 0      TMA producer   Q tiles once per item, K/V tiles into a ring of kSlots smem slots
@@ -12,8 +12,14 @@
 //   warps 4-7   softmax for query tile 0 (one thread per row): online softmax in fp32, lazy rescale of O,
 //   warps 8-11  softmax for query tile 1                        P written back to TMEM as bf16, epilogue
 // TMEM (512 columns): S0 [0,128) / P0 aliases [0,64); S1 [128,256) / P1; O0 [256,256+D); O1 [256+D,256+2D).
-// Issue order  S0(0) S1(0) | PV0(j) S0(j+1) PV1(j) S1(j+1) | ...  keeps the tensor pipe busy while the
-// other tile's softmax runs (two-tile ping-pong).
+// Issue order  S0(0) S1(0) | PV0(j) S0(j+1) PV1(j) S1(j+1) | ...  keeps the tensor pipe busy while the other
+// tile's softmax runs (two-tile ping-pong); P is handed over in two 64-key halves so that the first half of
+// O += P V runs under the second half of the exponentials.
+//
+// Cluster: the host gives the two CTAs of a cluster two items of the SAME (session, head) wherever it can.  Each
+// CTA then loads half of every K/V tile and multicasts it to both (one L2 read per pair of CTAs); both CTAs cycle
+// the same number of tiles through their rings so that a tile sits at the same smem offset in both.  Every slot
+// release goes to the kv_empty barriers of both CTAs (count 2), also when the two CTAs work on unrelated items.
 #include "internal.h"
 #include "ptx.cuh"
 
