@@ -513,3 +513,12 @@ def test_config4_churn_full_size():
           f"attention {np.sum(flops) / np.sum(lat_a) / 1e9:.0f} TFLOP/s over the run (best step {tfl.max():.0f}); "
           f"offload {off_bytes / 1e9:.1f} GB in {off_ms:.0f} ms = {off_bytes / max(off_ms, 1e-9) / 1e6:.1f} GB/s")
     dp.g.close()
+
+
+# ---- latency model l_hat(n): the sweep runs through the C ABI and is monotone in n ---------
+def test_latency_model_sweep_small():
+    from paper_2606_19271_b200 import latency_model
+    rows = [latency_model.measure(n, 6, 4, 128, 520, 21, 256, reps=3) for n in (1, 4)]
+    for attn_ms, app_ms, tfl in rows:
+        assert attn_ms > 0 and app_ms > 0 and tfl > 0
+    assert rows[1][0] > rows[0][0]          # four sessions take longer than one
