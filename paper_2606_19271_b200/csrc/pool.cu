@@ -93,6 +93,7 @@ struct Session {
   std::vector<int32_t> host_slots;  // arena slots holding the pages while SUSPENDED (logical order)
   uint64_t compute_seq = 0;         // last compute-stream call that touched the session
   uint64_t side_seq = 0;            // last side-stream copy that touched the session
+  uint64_t ver = 0;                 // new value whenever P, o or pt change (keys the attention schedule cache)
 };
 
 struct Staging {      // pinned host + device buffer pair for per-call schedule records
@@ -134,6 +135,14 @@ struct ts_pool {
   size_t stage_cap = 0;
   int64_t launches = 0;
   std::vector<int32_t> scratch_mark;       // duplicate detection
+  // attention schedule of the last batch (a1), reused while the batch and its sessions' page tables are unchanged:
+  // every layer and denoising pass of one chunk step then pays the scheduler once
+  uint64_t ver_seq = 0;                    // source of Session::ver values (never repeats, also across reopen)
+  std::vector<int64_t> sched_key;
+  std::vector<tc::SessDesc> sched_sess;
+  std::vector<int32_t> sched_pt, sched_cta;
+  std::vector<tc::WorkItem> sched_items;
+  int64_t sched_builds = 0;
 };
 
 namespace tc {
@@ -382,6 +391,7 @@ int ts_session_open(ts_pool* pool, int32_t* sid_out) {
       Session& s = pool->sess[i];
       s = Session();
       s.state = TS_SESSION_RESIDENT;
+      s.ver = ++pool->ver_seq;
       *sid_out = i;
       return TS_OK;
     }
@@ -469,165 +479,181 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   TS_CUDA(cudaSetDevice(c.device));
   const int T = c.frame_tokens, H = c.n_heads, D = c.head_dim, W = c.window_frames;
 
-  // ---- a1: collect + coalesce
-  size_t n_pt_total = 0;
-  int n_items = 0;
+  // ---- a1: collect + coalesce.  The schedule (session descriptors, packed page tables, work items per CTA) depends
+  // only on the batch and on its sessions' page-table state, so it is built once and reused by every later call with
+  // the same key - all layers and denoising passes of a chunk step; only the Q/K/V tensor maps are encoded per call.
+  std::vector<int64_t> key;
+  key.reserve(3 * (size_t)n + 1);
+  key.push_back(n);
   for (int b = 0; b < n; ++b) {
-    n_pt_total += pool->sess[sids[b]].pt.size();
-    n_items += H * ((chunk_frames[b] * T + 255) / 256);
+    key.push_back(sids[b]);
+    key.push_back(chunk_frames[b]);
+    key.push_back((int64_t)pool->sess[sids[b]].ver);
   }
-  // items are dealt to CTA pairs (2-CTA clusters): at most one cluster item per candidate, two CTA entries each
-  n_items *= 2;
   const int grid_max = std::max(2, pool->sm_count & ~1);
+  if (key != pool->sched_key) {
+    ++pool->sched_builds;
+    std::vector<SessDesc>& sd = pool->sched_sess;
+    std::vector<int32_t>& pt = pool->sched_pt;
+    std::vector<int32_t>& cta_begin = pool->sched_cta;
+    std::vector<WorkItem>& items = pool->sched_items;
+    sd.assign(n, SessDesc());
+    pt.clear();
+    struct Cand {
+      int cost, sess, head, q_pair, n_kv;
+    };
+    std::vector<Cand> cands;
+    int q_off = 0;
+    for (int b = 0; b < n; ++b) {
+      const Session& s = pool->sess[sids[b]];
+      const int cfr = chunk_frames[b];
+      const int C = cfr * T;
+      const int a = W > 0 ? std::max(0, s.P + cfr - W) : 0;     // window start in frames (R6 i)
+      SessDesc& d = sd[b];
+      d.q_off = q_off;
+      d.C = C;
+      d.x_begin = s.o + a * T;
+      d.x_end = s.o + s.P * T;
+      d.pt_off = (int32_t)pt.size();
+      d.n_pt = (int32_t)s.pt.size();
+      d.pad0 = d.pad1 = 0;
+      pt.insert(pt.end(), s.pt.begin(), s.pt.end());
+      const int n_pairs = (C + 255) / 256;
+      for (int qp = 0; qp < n_pairs; ++qp) {
+        int n_q, n_kv;
+        item_geometry(c, C, d.x_begin, d.x_end, qp, &n_q, &n_kv);
+        // time model in twentieths of a two-tile KV step, fitted to per-CTA cycle counts on configs[2]
+        // (3184 clk per step + 14.7 k clk per item): 4.5 steps per item for the Q load, pipeline fill and epilogue.
+        // A lone query tile has no ping-pong partner to hide its S -> softmax -> PV chain behind: ~0.95 of a pair step.
+        const int cost = (n_q == 2 ? 20 : 19) * n_kv + 90;
+        for (int h = 0; h < H; ++h) cands.push_back({cost, b, h, qp, n_kv});
+      }
+      q_off += C;
+    }
+    // ---- cluster items.  The q-pair items of one (session, head) stream read the same K/V pages: two of them at a
+    // time go to the two CTAs of a cluster, which then load half of every K/V tile each and multicast it to both
+    // (mc).  A stream's odd item out is paired with another stream's (or with nothing): those two share a cluster
+    // without sharing loads.  Both CTAs cycle max(n_kv) tiles through their smem rings so that they stay on the same
+    // ring position.
+    struct CItem {
+      int cost;
+      int64_t stream_cost;
+      int stream;
+      Cand a, b;       // b.q_pair < 0: no second item
+      bool mc;
+    };
+    std::vector<int64_t> stream_cost((size_t)n * H, 0);
+    for (const Cand& x : cands) stream_cost[(size_t)x.sess * H + x.head] += x.cost;
+    // within a stream: by KV length (longest first), two-tile items before a lone tile
+    std::stable_sort(cands.begin(), cands.end(), [&](const Cand& x, const Cand& y) {
+      const size_t sx = (size_t)x.sess * H + x.head, sy = (size_t)y.sess * H + y.head;
+      if (sx != sy) return sx < sy;
+      if (x.n_kv != y.n_kv) return x.n_kv > y.n_kv;
+      return x.cost > y.cost;
+    });
+    std::vector<CItem> citems;
+    std::vector<Cand> odd;
+    for (size_t i = 0; i < cands.size();) {
+      size_t e = i;
+      while (e < cands.size() && cands[e].sess == cands[i].sess && cands[e].head == cands[i].head) ++e;
+      const int stream = cands[i].sess * H + cands[i].head;
+      // pair items of EQUAL KV length first (neither CTA then waits for tiles only its partner needs); what is left
+      // over (at most one item per length) is paired in length order, and the stream's last odd item goes to `odd`
+      std::vector<Cand> rest;
+      while (i < e) {
+        if (i + 1 < e && cands[i].n_kv == cands[i + 1].n_kv) {
+          citems.push_back({std::max(cands[i].cost, cands[i + 1].cost), stream_cost[stream], stream, cands[i], cands[i + 1], true});
+          i += 2;
+        } else {
+          rest.push_back(cands[i++]);
+        }
+      }
+      size_t r = 0;
+      for (; r + 1 < rest.size(); r += 2)
+        citems.push_back({std::max(rest[r].cost, rest[r + 1].cost), stream_cost[stream], stream, rest[r], rest[r + 1], true});
+      if (r < rest.size()) odd.push_back(rest[r]);
+    }
+    std::stable_sort(odd.begin(), odd.end(), [](const Cand& x, const Cand& y) { return x.cost > y.cost; });
+    for (size_t i = 0; i < odd.size(); i += 2) {
+      Cand none = odd[i];
+      none.q_pair = -1;
+      none.n_kv = 0;
+      none.cost = 0;
+      const Cand& second = (i + 1 < odd.size()) ? odd[i + 1] : none;
+      const int stream = odd[i].sess * H + odd[i].head;
+      citems.push_back({std::max(odd[i].cost, second.cost), stream_cost[stream], stream, odd[i], second, false});
+    }
+    // List scheduling in stream order, heaviest streams first (LPT at stream granularity, so that the tail of the
+    // schedule is made of short items): a stream's items are dealt out back to back, each to the least-loaded
+    // cluster, and run at the same time - the stream's K/V then comes from DRAM once and from L2 afterwards.
+    std::stable_sort(citems.begin(), citems.end(), [](const CItem& x, const CItem& y) {
+      if (x.stream_cost != y.stream_cost) return x.stream_cost > y.stream_cost;
+      if (x.stream != y.stream) return x.stream < y.stream;
+      return x.cost > y.cost;
+    });
+    const int n_clusters = std::min(grid_max / 2, (int)citems.size());
+    const int grid = 2 * n_clusters;
+    std::vector<std::vector<int>> per_cluster(n_clusters);
+    {
+      typedef std::pair<int64_t, int> Load;   // (load, cluster)
+      std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
+      for (int i = 0; i < n_clusters; ++i) heap.push({0, i});
+      for (int i = 0; i < (int)citems.size(); ++i) {
+        Load top = heap.top();
+        heap.pop();
+        per_cluster[top.second].push_back(i);
+        heap.push({top.first + citems[i].cost, top.second});
+      }
+    }
+
+    cta_begin.assign(grid + 1, 0);
+    items.clear();
+    for (int ci = 0; ci < grid; ++ci) {
+      cta_begin[ci] = (int32_t)items.size();
+      for (int i : per_cluster[ci >> 1]) {
+        const CItem& it = citems[i];
+        const Cand& x = (ci & 1) ? it.b : it.a;
+        WorkItem wi;
+        wi.sess = x.sess;
+        wi.head = x.head;
+        wi.q_pair = x.q_pair;
+        wi.pipe = (uint32_t)std::max(it.a.n_kv, it.b.n_kv) | (it.mc ? 0x80000000u : 0u);
+        items.push_back(wi);
+      }
+    }
+    cta_begin[grid] = (int32_t)items.size();
+    pool->sched_key = key;
+  }
+  const int grid = (int)pool->sched_cta.size() - 1;
   ScheduleLayout L;
-  L.n_items = n_items;
-  L.grid = grid_max;
+  L.n_items = (int)pool->sched_items.size();
+  L.grid = grid;
   L.off_maps = 0;
   L.off_sess = align_up(L.off_maps + (size_t)n * 3 * sizeof(CUtensorMap), 128);
   L.off_pt = align_up(L.off_sess + (size_t)n * sizeof(SessDesc), 128);
-  L.off_cta = align_up(L.off_pt + n_pt_total * 4, 128);
-  L.off_items = align_up(L.off_cta + (size_t)(grid_max + 1) * 4, 128);
-  L.bytes = L.off_items + (size_t)n_items * sizeof(WorkItem);
+  L.off_cta = align_up(L.off_pt + pool->sched_pt.size() * 4, 128);
+  L.off_items = align_up(L.off_cta + (size_t)(grid + 1) * 4, 128);
+  L.bytes = L.off_items + pool->sched_items.size() * sizeof(WorkItem);
   Staging* st = nullptr;
   rc = acquire_staging(pool, L.bytes, &st);
   if (rc != TS_OK) return rc;
   CUtensorMap* maps = reinterpret_cast<CUtensorMap*>(st->h + L.off_maps);
-  SessDesc* sd = reinterpret_cast<SessDesc*>(st->h + L.off_sess);
-  int32_t* pt = reinterpret_cast<int32_t*>(st->h + L.off_pt);
-  int32_t* cta_begin = reinterpret_cast<int32_t*>(st->h + L.off_cta);
-  WorkItem* items = reinterpret_cast<WorkItem*>(st->h + L.off_items);
-
-  struct Cand {
-    int cost, sess, head, q_pair, n_kv;
-  };
-  std::vector<Cand> cands;
-  cands.reserve(n_items);
-  int q_off = 0, pt_off = 0;
+  memcpy(st->h + L.off_sess, pool->sched_sess.data(), (size_t)n * sizeof(SessDesc));
+  memcpy(st->h + L.off_pt, pool->sched_pt.data(), pool->sched_pt.size() * 4);
+  memcpy(st->h + L.off_cta, pool->sched_cta.data(), (size_t)(grid + 1) * 4);
+  memcpy(st->h + L.off_items, pool->sched_items.data(), pool->sched_items.size() * sizeof(WorkItem));
   for (int b = 0; b < n; ++b) {
-    const Session& s = pool->sess[sids[b]];
-    const int cfr = chunk_frames[b];
-    const int C = cfr * T;
-    const int a = W > 0 ? std::max(0, s.P + cfr - W) : 0;     // window start in frames (R6 i)
-    SessDesc& d = sd[b];
-    d.q_off = q_off;
-    d.C = C;
-    d.x_begin = s.o + a * T;
-    d.x_end = s.o + s.P * T;
-    d.pt_off = pt_off;
-    d.n_pt = (int32_t)s.pt.size();
-    d.pad0 = d.pad1 = 0;
-    std::copy(s.pt.begin(), s.pt.end(), pt + pt_off);
     // per-session 3D maps {D, H, C}: rows past the session's chunk read as zeros, never as a neighbour's tokens
-    const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)H, (cuuint64_t)C};
+    const SessDesc& d = pool->sched_sess[b];
+    const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)H, (cuuint64_t)d.C};
     const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)H * D * 2};
     const cuuint32_t box_q[3] = {64, 1, 128};
     const cuuint32_t box_kv[3] = {64, 1, (cuuint32_t)std::min(c.page_tokens, 64)};   // same box rows as the cache maps
-    const size_t byte_off = (size_t)q_off * H * D * 2;
+    const size_t byte_off = (size_t)d.q_off * H * D * 2;
     if (!encode_map(&maps[b * 3 + 0], (uint8_t*)q + byte_off, 3, dims, strides, box_q)) return TS_ERR_CUDA;
     if (!encode_map(&maps[b * 3 + 1], (uint8_t*)k + byte_off, 3, dims, strides, box_kv)) return TS_ERR_CUDA;
     if (!encode_map(&maps[b * 3 + 2], (uint8_t*)v + byte_off, 3, dims, strides, box_kv)) return TS_ERR_CUDA;
-    const int n_pairs = (C + 255) / 256;
-    for (int qp = 0; qp < n_pairs; ++qp) {
-      int n_q, n_kv;
-      item_geometry(c, C, d.x_begin, d.x_end, qp, &n_q, &n_kv);
-      // time model in twentieths of a two-tile KV step, fitted to per-CTA cycle counts on configs[2]
-      // (3184 clk per step + 14.7 k clk per item): 4.5 steps per item for the Q load, pipeline fill and epilogue.
-      // A lone query tile has no ping-pong partner to hide its S -> softmax -> PV chain behind: ~0.95 of a pair step.
-      const int cost = (n_q == 2 ? 20 : 19) * n_kv + 90;
-      for (int h = 0; h < H; ++h) cands.push_back({cost, b, h, qp, n_kv});
-    }
-    q_off += C;
-    pt_off += (int)s.pt.size();
   }
-  // ---- cluster items.  The q-pair items of one (session, head) stream read the same K/V pages: two of them at a
-  // time go to the two CTAs of a cluster, which then load half of every K/V tile each and multicast it to both
-  // (mc).  A stream's odd item out is paired with another stream's (or with nothing): those two share a cluster
-  // without sharing loads.  Both CTAs cycle max(n_kv) tiles through their smem rings so that they stay on the same
-  // ring position.
-  struct CItem {
-    int cost;
-    int64_t stream_cost;
-    int stream;
-    Cand a, b;       // b.q_pair < 0: no second item
-    bool mc;
-  };
-  std::vector<int64_t> stream_cost((size_t)n * H, 0);
-  for (const Cand& x : cands) stream_cost[(size_t)x.sess * H + x.head] += x.cost;
-  // within a stream: by KV length (longest first), two-tile items before a lone tile
-  std::stable_sort(cands.begin(), cands.end(), [&](const Cand& x, const Cand& y) {
-    const size_t sx = (size_t)x.sess * H + x.head, sy = (size_t)y.sess * H + y.head;
-    if (sx != sy) return sx < sy;
-    if (x.n_kv != y.n_kv) return x.n_kv > y.n_kv;
-    return x.cost > y.cost;
-  });
-  std::vector<CItem> citems;
-  std::vector<Cand> odd;
-  for (size_t i = 0; i < cands.size();) {
-    size_t e = i;
-    while (e < cands.size() && cands[e].sess == cands[i].sess && cands[e].head == cands[i].head) ++e;
-    const int stream = cands[i].sess * H + cands[i].head;
-    // pair items of EQUAL KV length first (neither CTA then waits for tiles only its partner needs); what is left
-    // over (at most one item per length) is paired in length order, and the stream's last odd item goes to `odd`
-    std::vector<Cand> rest;
-    while (i < e) {
-      if (i + 1 < e && cands[i].n_kv == cands[i + 1].n_kv) {
-        citems.push_back({std::max(cands[i].cost, cands[i + 1].cost), stream_cost[stream], stream, cands[i], cands[i + 1], true});
-        i += 2;
-      } else {
-        rest.push_back(cands[i++]);
-      }
-    }
-    size_t r = 0;
-    for (; r + 1 < rest.size(); r += 2)
-      citems.push_back({std::max(rest[r].cost, rest[r + 1].cost), stream_cost[stream], stream, rest[r], rest[r + 1], true});
-    if (r < rest.size()) odd.push_back(rest[r]);
-  }
-  std::stable_sort(odd.begin(), odd.end(), [](const Cand& x, const Cand& y) { return x.cost > y.cost; });
-  for (size_t i = 0; i < odd.size(); i += 2) {
-    Cand none = odd[i];
-    none.q_pair = -1;
-    none.n_kv = 0;
-    none.cost = 0;
-    const Cand& second = (i + 1 < odd.size()) ? odd[i + 1] : none;
-    const int stream = odd[i].sess * H + odd[i].head;
-    citems.push_back({std::max(odd[i].cost, second.cost), stream_cost[stream], stream, odd[i], second, false});
-  }
-  // List scheduling in stream order, heaviest streams first (LPT at stream granularity, so that the tail of the
-  // schedule is made of short items): a stream's items are dealt out back to back, each to the least-loaded
-  // cluster, and run at the same time - the stream's K/V then comes from DRAM once and from L2 afterwards.
-  std::stable_sort(citems.begin(), citems.end(), [](const CItem& x, const CItem& y) {
-    if (x.stream_cost != y.stream_cost) return x.stream_cost > y.stream_cost;
-    if (x.stream != y.stream) return x.stream < y.stream;
-    return x.cost > y.cost;
-  });
-  const int n_clusters = std::min(grid_max / 2, (int)citems.size());
-  const int grid = 2 * n_clusters;
-  std::vector<std::vector<int>> per_cluster(n_clusters);
-  {
-    typedef std::pair<int64_t, int> Load;   // (load, cluster)
-    std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
-    for (int i = 0; i < n_clusters; ++i) heap.push({0, i});
-    for (int i = 0; i < (int)citems.size(); ++i) {
-      Load top = heap.top();
-      heap.pop();
-      per_cluster[top.second].push_back(i);
-      heap.push({top.first + citems[i].cost, top.second});
-    }
-  }
-  int w = 0;
-  for (int ci = 0; ci < grid; ++ci) {
-    cta_begin[ci] = w;
-    for (int i : per_cluster[ci >> 1]) {
-      const CItem& it = citems[i];
-      const Cand& x = (ci & 1) ? it.b : it.a;
-      items[w].sess = x.sess;
-      items[w].head = x.head;
-      items[w].q_pair = x.q_pair;
-      items[w].pipe = (uint32_t)std::max(it.a.n_kv, it.b.n_kv) | (it.mc ? 0x80000000u : 0u);
-      ++w;
-    }
-  }
-  cta_begin[grid] = w;
 
   // ---- ordering: wait (stream-side) for pending resumes of the batch's sessions
   for (int b = 0; b < n; ++b) TS_CUDA(pool->tl_side.wait(stream, pool->sess[sids[b]].side_seq));
@@ -699,6 +725,7 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, c
   int tok_off = 0, pt_off = 0, row_off = 0;
   for (int b = 0; b < n; ++b) {
     Session& s = pool->sess[sids[b]];
+    if (need[b] > 0) s.ver = ++pool->ver_seq;
     for (int i = 0; i < need[b]; ++i) {
       const int32_t pg = pool->free_q.front();
       pool->free_q.pop_front();
@@ -751,6 +778,7 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, c
     Session& s = pool->sess[sids[b]];
     s.compute_seq = seq;
     if (flags & TS_COMMIT) {
+      s.ver = ++pool->ver_seq;
       s.P += chunk_frames[b];
       const int e = W > 0 ? std::max(0, s.P - W) : 0;   // a4: evict oldest whole frames (R6 ii, R10)
       s.P -= e;
@@ -872,6 +900,7 @@ int ts_session_resume(ts_pool* pool, int32_t sid) {
   s.side_seq = pool->tl_side.record(pool->side);
   for (auto it = s.host_slots.rbegin(); it != s.host_slots.rend(); ++it) pool->host_free.push_back(*it);
   s.host_slots.clear();
+  s.ver = ++pool->ver_seq;
   s.state = TS_SESSION_RESIDENT;
   return TS_OK;
 }
