@@ -155,8 +155,13 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*
 /*
  * One coalesced chunk step with HOST buffers (the end-to-end entry point): copies q,k,v from (pinned) host
  * memory to device staging owned by the pool, runs ts_chunk_attention and ts_kv_append(flags) on
- * `cuda_stream`, copies `out` back to out_host.  All copies are enqueued on `cuda_stream`; the call returns
- * without waiting.  Staging grows on demand (cudaMalloc) and is reused.
+ * `cuda_stream`, copies `out` back to out_host.  The call returns without waiting.
+ *   q_host, k_host, v_host : host bf16 [sum_b C_b][H][D] (pinned for asynchronous copies).  They are read by a copy
+ *       stream of the pool that does NOT wait for `cuda_stream`: the contents must be valid when the call is made
+ *       and stay unchanged until `cuda_stream` has passed the call.  That is what lets the input copy of one call
+ *       run under the attention and the output copy of the previous one (two staging sets).
+ *   out_host : host bf16, same shape; complete once `cuda_stream` has passed the call (stream order).
+ * Staging grows on demand (cudaMalloc, with a device synchronisation) and is reused.  Errors as the two calls.
  */
 int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
                        const void* q_host, const void* k_host, const void* v_host, void* out_host,

@@ -131,7 +131,10 @@ struct ts_pool {
   static constexpr int kRing = 8;
   Staging ring[kRing];
   int ring_next = 0;
-  uint8_t* stage_dev = nullptr;            // ts_chunk_step_host: device staging for q,k,v,out
+  uint8_t* stage_dev = nullptr;            // ts_chunk_step_host: two device staging sets for q,k,v,out
+  cudaStream_t h2d_s = nullptr, d2h_s = nullptr;   // ... its copy streams (input of step t+1 overlaps step t)
+  cudaEvent_t ev_in = nullptr, ev_attn = nullptr, ev_out = nullptr, ev_free[2] = {nullptr, nullptr};
+  uint64_t host_steps = 0;
   size_t stage_cap = 0;
   int64_t launches = 0;
   std::vector<int32_t> scratch_mark;       // duplicate detection
@@ -284,6 +287,10 @@ int ts_pool_destroy(ts_pool* pool) {
     if (s.ev) cudaEventDestroy(s.ev);
   }
   if (pool->stage_dev) cudaFree(pool->stage_dev);
+  if (pool->h2d_s) cudaStreamDestroy(pool->h2d_s);
+  if (pool->d2h_s) cudaStreamDestroy(pool->d2h_s);
+  for (cudaEvent_t e : {pool->ev_in, pool->ev_attn, pool->ev_out, pool->ev_free[0], pool->ev_free[1]})
+    if (e) cudaEventDestroy(e);
   pool->tl_compute.destroy();
   pool->tl_side.destroy();
   if (pool->own_side && pool->side) cudaStreamDestroy(pool->side);
@@ -927,28 +934,51 @@ int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   int64_t tokens = 0;
   for (int b = 0; b < n; ++b) tokens += (int64_t)chunk_frames[b] * c.frame_tokens;
   const size_t tensor_bytes = align_up((size_t)tokens * c.n_heads * c.head_dim * 2, 1024);
-  if (pool->stage_cap < 4 * tensor_bytes) {
+  if (pool->h2d_s == nullptr) {
+    TS_CUDA(cudaStreamCreateWithFlags(&pool->h2d_s, cudaStreamNonBlocking));
+    TS_CUDA(cudaStreamCreateWithFlags(&pool->d2h_s, cudaStreamNonBlocking));
+    for (cudaEvent_t* e : {&pool->ev_in, &pool->ev_attn, &pool->ev_out, &pool->ev_free[0], &pool->ev_free[1]})
+      TS_CUDA(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+  }
+  if (pool->stage_cap < 8 * tensor_bytes) {
     if (pool->stage_dev) {
       TS_CUDA(cudaDeviceSynchronize());
       TS_CUDA(cudaFree(pool->stage_dev));
       pool->stage_dev = nullptr;
       pool->stage_cap = 0;
     }
-    TS_CUDA(cudaMalloc((void**)&pool->stage_dev, 4 * tensor_bytes));
-    pool->stage_cap = 4 * tensor_bytes;
+    TS_CUDA(cudaMalloc((void**)&pool->stage_dev, 8 * tensor_bytes));
+    pool->stage_cap = 8 * tensor_bytes;
+    pool->host_steps = 0;
   }
-  uint8_t* dq = pool->stage_dev;
+  // Two staging sets and two copy streams: the H2D of this call does not wait for the caller's stream (host buffers
+  // are read like any pinned cudaMemcpyAsync source: valid from the call until the stream reaches the end of the
+  // call), only for the staging set to be free, so it runs under the attention and the D2H of the previous call.
+  const int slot = (int)(pool->host_steps & 1);
+  const bool slot_used = pool->host_steps >= 2;
+  ++pool->host_steps;
+  uint8_t* dq = pool->stage_dev + (size_t)slot * (pool->stage_cap / 2);
   uint8_t* dk = dq + tensor_bytes;
   uint8_t* dv = dk + tensor_bytes;
   uint8_t* dout = dv + tensor_bytes;
   const size_t nbytes = (size_t)tokens * c.n_heads * c.head_dim * 2;
-  TS_CUDA(cudaMemcpyAsync(dq, q_host, nbytes, cudaMemcpyHostToDevice, stream));
-  TS_CUDA(cudaMemcpyAsync(dk, k_host, nbytes, cudaMemcpyHostToDevice, stream));
-  TS_CUDA(cudaMemcpyAsync(dv, v_host, nbytes, cudaMemcpyHostToDevice, stream));
+  if (slot_used) TS_CUDA(cudaStreamWaitEvent(pool->h2d_s, pool->ev_free[slot], 0));
+  TS_CUDA(cudaMemcpyAsync(dq, q_host, nbytes, cudaMemcpyHostToDevice, pool->h2d_s));
+  TS_CUDA(cudaMemcpyAsync(dk, k_host, nbytes, cudaMemcpyHostToDevice, pool->h2d_s));
+  TS_CUDA(cudaMemcpyAsync(dv, v_host, nbytes, cudaMemcpyHostToDevice, pool->h2d_s));
+  TS_CUDA(cudaEventRecord(pool->ev_in, pool->h2d_s));
+  TS_CUDA(cudaStreamWaitEvent(stream, pool->ev_in, 0));
   rc = ts_chunk_attention(pool, layer, n, sids, chunk_frames, dq, dk, dv, dout, nullptr, scale, cuda_stream);
   if (rc != TS_OK) return rc;
-  TS_CUDA(cudaMemcpyAsync(out_host, dout, nbytes, cudaMemcpyDeviceToHost, stream));
-  return ts_kv_append(pool, layer, n, sids, chunk_frames, dk, dv, flags, cuda_stream);
+  TS_CUDA(cudaEventRecord(pool->ev_attn, stream));
+  TS_CUDA(cudaStreamWaitEvent(pool->d2h_s, pool->ev_attn, 0));
+  TS_CUDA(cudaMemcpyAsync(out_host, dout, nbytes, cudaMemcpyDeviceToHost, pool->d2h_s));
+  TS_CUDA(cudaEventRecord(pool->ev_out, pool->d2h_s));
+  rc = ts_kv_append(pool, layer, n, sids, chunk_frames, dk, dv, flags, cuda_stream);
+  if (rc != TS_OK) return rc;
+  TS_CUDA(cudaStreamWaitEvent(stream, pool->ev_out, 0));   // stream order: out_host is complete when the call is
+  TS_CUDA(cudaEventRecord(pool->ev_free[slot], stream));   // ... and the staging set is free again
+  return TS_OK;
 }
 
 }  // extern "C"

@@ -522,3 +522,35 @@ def test_latency_model_sweep_small():
     for attn_ms, app_ms, tfl in rows:
         assert attn_ms > 0 and app_ms > 0 and tfl > 0
     assert rows[1][0] > rows[0][0]          # four sessions take longer than one
+
+
+# ---- ts_chunk_step_host: the host-buffer entry point (H2D, attention, append, D2H), two pipelined steps ------------
+def test_chunk_step_host_two_steps():
+    from paper_2606_19271_b200 import TS_COMMIT
+    shape = shape_of(n_heads=3, head_dim=128, frame_tokens=200, window_frames=6, page_tokens=64, n_pages=96)
+    rng = np.random.default_rng(11)
+    dp = DualPool(shape, rng.permutation(shape.n_pages))
+    T = shape.frame_tokens
+    sids = [dp.open(), dp.open()]
+    k0, v0 = draw(rng, 2 * T, shape), draw(rng, 2 * T, shape)
+    dp.append(0, [sids[1]], [2], k0, v0)
+    outs, refs = [], []
+    hosts = []
+    for step in range(3):                      # three steps back to back: both staging sets are reused
+        cf = [2, 1]
+        n_tok = sum(cf) * T
+        q, k, v = (draw(rng, n_tok, shape) for _ in range(3))
+        o_ref, _ = oracle.chunk_attention(dp.o, 0, sids, cf, q, k, v, scale_of(shape))
+        hq, hk, hv = (torch.from_numpy(x.view(np.int16)).pin_memory() for x in (q, k, v))
+        hout = torch.zeros_like(hq).pin_memory()
+        hosts.append((hq, hk, hv, hout))       # keep the host buffers alive until the stream is done
+        dp.g.ts_chunk_step_host(0, sids, cf, hq, hk, hv, hout, float(scale_of(shape)), TS_COMMIT)
+        dp.o.append(0, sids, cf, k, v, commit=True)
+        refs.append(o_ref)
+    torch.cuda.synchronize()
+    for (hq, hk, hv, hout), o_ref in zip(hosts, refs):
+        o_gpu = hout.view(torch.bfloat16).double().numpy()
+        assert np.abs(o_gpu - o_ref).max() <= 2e-2
+        assert rel_l2(o_gpu, o_ref) <= 5e-3
+    dp.check_state(sids, kv=True)
+    dp.g.close()
