@@ -554,3 +554,32 @@ def test_chunk_step_host_two_steps():
         assert rel_l2(o_gpu, o_ref) <= 5e-3
     dp.check_state(sids, kv=True)
     dp.g.close()
+
+
+# ---- cluster scheduling edge cases: the two CTAs of a cluster share K/V loads of one (session, head) stream ---------
+@pytest.mark.parametrize("n_heads,priors,chunks", [
+    (1, [0], [3]),            # one stream, q-pair KV lengths 3,5,8,8 tiles: an equal pair + a mismatched multicast pair
+    (1, [2], [1]),            # one stream, two q-pairs of different length: one mismatched pair, nothing else
+    (1, [0], [4]),            # 5 q-pairs: pairs + one odd item that shares a cluster with nothing
+    (3, [0, 4, 1], [3, 2, 4]),   # odd items of different streams share clusters without sharing loads
+    (2, [5], [1]),            # rolled window (head offset != 0), lone query tiles only
+])
+def test_cluster_pairing_shapes(n_heads, priors, chunks):
+    shape = shape_of(n_heads=n_heads, head_dim=128, frame_tokens=300, window_frames=5, page_tokens=64,
+                     n_pages=160, max_sessions=4)
+    rng = np.random.default_rng(1000 + n_heads + sum(priors) + 7 * sum(chunks))
+    dp = DualPool(shape, rng.permutation(shape.n_pages))
+    T = shape.frame_tokens
+    sids = [dp.open() for _ in priors]
+    for sid, P in zip(sids, priors):
+        if P:
+            dp.feed_prior(sid, [draw(rng, P * T, shape)], [draw(rng, P * T, shape)])
+    total = sum(chunks) * T
+    for rep in range(2):      # the second call reuses the cached schedule
+        q, k, v = (draw(rng, total, shape) for _ in range(3))
+        dp.attention(0, sids, chunks, q, k, v, scale_of(shape))
+    dp.append(0, sids, chunks, k, v)
+    dp.check_state(sids)
+    q, k, v = (draw(rng, total, shape) for _ in range(3))
+    dp.attention(0, sids, [min(c, 2) for c in chunks], *(x[:sum(min(c, 2) for c in chunks) * T] for x in (q, k, v)),
+                 scale_of(shape))
