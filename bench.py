@@ -6,12 +6,13 @@
 One JSON line on stdout (rank 0).  A "step" is one pass of the hot path over one coalesced batch:
     resume(idle session X) on the side stream                      (a6)
     open + close of a transient session                            (a7)
-    ts_chunk_attention(batch of 8)        scheduler + attention    (a1, a2)
-    ts_kv_append(batch of 8, flags=0)     paged scatter            (a3)
+    ts_chunk_step(batch of 8, flags=0)    scheduler + attention (a1, a2) and paged scatter (a3), the scatter
+                                          running under the attention kernel on a stream of the pool
     suspend(X) on the side stream                                  (a5)
 flags=0 keeps every timed step on the identical drawn state of configs[2]; the window roll (a4) is host
 integer arithmetic inside ts_kv_append(TS_COMMIT), exercised by the tests, not by the timed loop.
-`value` = attention FLOPs of the batch / step time (all ranks), `roofline` is the attention kernel alone,
+`value` = attention FLOPs of the batch / step time (all ranks); `roofline` (attention) and `append` are the two
+kernels timed alone with CUDA events, one after the other, in a second loop over the same steps;
 `e2e` is the same step through ts_chunk_step_host with pinned HOST buffers (H2D of Q/K/V and D2H of O inside
 the timed region).  N > 1 runs N independent replicas (sessions are independent units).
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
@@ -172,20 +173,25 @@ def build_workload(device, with_oracle):
             "x": x, "x_pages": pool.ts_session_info(x)["n_pages"], "chunks": chunks, "to_bits": to_bits}
 
 
-def step_device(wl, out, ev=None):
+def step_device(wl, out):
     """One coalesced chunk step, inputs resident in HBM."""
     pool = wl["pool"]
     pool.ts_session_resume(wl["x"])
     t = pool.ts_session_open()
     pool.ts_session_close(t)
-    if ev is not None:
-        ev[0].record()
+    pool.ts_chunk_step(0, wl["sids"], wl["cf"], wl["q"], wl["k"], wl["v"], out, None, float(wl["w"].scale), 0)
+    pool.ts_session_suspend(wl["x"])
+
+
+def step_kernels(wl, out, ev):
+    """The same step with attention and append as separate calls on one stream, for per-kernel timing."""
+    pool = wl["pool"]
+    pool.ts_session_resume(wl["x"])
+    ev[0].record()
     pool.ts_chunk_attention(0, wl["sids"], wl["cf"], wl["q"], wl["k"], wl["v"], out, None, float(wl["w"].scale))
-    if ev is not None:
-        ev[1].record()
+    ev[1].record()
     pool.ts_kv_append(0, wl["sids"], wl["cf"], wl["k"], wl["v"], 0)
-    if ev is not None:
-        ev[2].record()
+    ev[2].record()
     pool.ts_session_suspend(wl["x"])
 
 
@@ -284,21 +290,36 @@ def main():
         step_device(wl, out)
         join_side(pool)
     barrier()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
     t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    step_evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
     launches0 = pool.ts_pool_launch_count()
     with ClockSampler(device.index if device.index is not None else 0) as clocks:
         t_begin.record()
         for i in range(args.steps):
-            step_device(wl, out, evs[i])
+            step_evs[i][0].record()
+            step_device(wl, out)
             join_side(pool)
+            step_evs[i][1].record()
         t_end.record()
         barrier()
     launches = pool.ts_pool_launch_count() - launches0
     ms_total = t_begin.elapsed_time(t_end)
+    step_ms_max = float(max(e[0].elapsed_time(e[1]) for e in step_evs))
+
+    # ---- the two kernels alone (same steps, attention and append as separate calls on one stream).  The GPU is
+    # power-capped: a short idle gap lets this loop start from the same power state as the timed loop above.
+    time.sleep(0.5)
+    for _ in range(args.warmup):
+        step_kernels(wl, out, [torch.cuda.Event(enable_timing=True) for _ in range(3)])
+        join_side(pool)
+    barrier()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    for i in range(args.steps):
+        step_kernels(wl, out, evs[i])
+        join_side(pool)
+    barrier()
     attn_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
     append_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
-    step_ms_max = float(max(evs[i][0].elapsed_time(evs[i][2]) for i in range(args.steps)))
 
     # ---- offload leg (side stream, timed alone): suspend / resume of a full-window session
     off = measure_offload(wl)

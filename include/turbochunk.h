@@ -153,6 +153,18 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*
                  void* cuda_stream);
 
 /*
+ * One coalesced chunk step with DEVICE buffers: ts_chunk_attention followed by ts_kv_append(flags) as one call
+ * (PAPER.md:66 (iii): "invokes the model once for the batch ... writes ... updated states back").  Results are those
+ * of the two calls in sequence.  The append writes cache slots this step's attention does not read (R5) and is
+ * HBM-bound while the attention is tensor-bound, so it runs on a stream of the pool UNDER the attention kernel;
+ * `cuda_stream` waits for both, and everything the pool remembers about completion is recorded on `cuda_stream`.
+ * Arguments as in the two calls.  All-or-nothing: page demand is checked before anything is enqueued.
+ */
+int ts_chunk_step(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*host*/,
+                  const int32_t* chunk_frames /*host*/, const void* q, const void* k, const void* v, void* out,
+                  float* lse, float scale, uint32_t flags, void* cuda_stream);
+
+/*
  * One coalesced chunk step with HOST buffers (the end-to-end entry point): copies q,k,v from (pinned) host
  * memory to device staging owned by the pool, runs ts_chunk_attention and ts_kv_append(flags) on
  * `cuda_stream`, copies `out` back to out_host.  The call returns without waiting.

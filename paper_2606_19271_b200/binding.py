@@ -18,7 +18,7 @@ TS_COMMIT = 1
 
 EXPORTED_SYMBOLS = [
     "ts_pool_page_bytes", "ts_pool_slab_bytes", "ts_pool_create", "ts_pool_destroy", "ts_session_open",
-    "ts_session_close", "ts_chunk_attention", "ts_kv_append", "ts_chunk_step_host", "ts_session_suspend",
+    "ts_session_close", "ts_chunk_attention", "ts_kv_append", "ts_chunk_step", "ts_chunk_step_host", "ts_session_suspend",
     "ts_session_resume", "ts_offload_sync", "ts_session_info", "ts_session_page_table", "ts_gather_kv",
     "ts_pool_free_list", "ts_pool_stats", "ts_pool_side_stream", "ts_pool_launch_count", "ts_strerror",
     "ts_last_cuda_error", "ts_version",
@@ -61,6 +61,7 @@ def _load():
     L.ts_session_close.argtypes = [P, C.c_int32]
     L.ts_chunk_attention.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, P, P, P, C.c_float, P]
     L.ts_kv_append.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, C.c_uint32, P]
+    L.ts_chunk_step.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, P, P, P, C.c_float, C.c_uint32, P]
     L.ts_chunk_step_host.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, P, P, C.c_float, C.c_uint32, P]
     L.ts_session_suspend.argtypes = [P, C.c_int32]
     L.ts_session_resume.argtypes = [P, C.c_int32]
@@ -178,6 +179,11 @@ class TurboChunkPool:
     def ts_kv_append(self, layer, sids, chunk_frames, k, v, flags=TS_COMMIT, stream=None):
         _check(lib.ts_kv_append(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(k), _ptr(v),
                                 C.c_uint32(flags), _stream(stream)), "ts_kv_append")
+
+    def ts_chunk_step(self, layer, sids, chunk_frames, q, k, v, out, lse=None, scale=1.0, flags=TS_COMMIT, stream=None):
+        _check(lib.ts_chunk_step(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(q), _ptr(k), _ptr(v),
+                                 _ptr(out), _ptr(lse), C.c_float(float(scale)), C.c_uint32(flags), _stream(stream)),
+               "ts_chunk_step")
 
     def ts_chunk_step_host(self, layer, sids, chunk_frames, q_host, k_host, v_host, out_host, scale, flags=TS_COMMIT,
                            stream=None):

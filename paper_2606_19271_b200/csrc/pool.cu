@@ -135,6 +135,8 @@ struct ts_pool {
   cudaStream_t h2d_s = nullptr, d2h_s = nullptr;   // ... its copy streams (input of step t+1 overlaps step t)
   cudaEvent_t ev_in = nullptr, ev_attn = nullptr, ev_out = nullptr, ev_free[2] = {nullptr, nullptr};
   uint64_t host_steps = 0;
+  cudaStream_t aux_s = nullptr;            // ts_chunk_step: the append runs here, under the attention kernel
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   size_t stage_cap = 0;
   int64_t launches = 0;
   std::vector<int32_t> scratch_mark;       // duplicate detection
@@ -289,6 +291,9 @@ int ts_pool_destroy(ts_pool* pool) {
   if (pool->stage_dev) cudaFree(pool->stage_dev);
   if (pool->h2d_s) cudaStreamDestroy(pool->h2d_s);
   if (pool->d2h_s) cudaStreamDestroy(pool->d2h_s);
+  if (pool->aux_s) cudaStreamDestroy(pool->aux_s);
+  if (pool->ev_fork) cudaEventDestroy(pool->ev_fork);
+  if (pool->ev_join) cudaEventDestroy(pool->ev_join);
   for (cudaEvent_t e : {pool->ev_in, pool->ev_attn, pool->ev_out, pool->ev_free[0], pool->ev_free[1]})
     if (e) cudaEventDestroy(e);
   pool->tl_compute.destroy();
@@ -692,8 +697,10 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
 }
 
 // --------------------------------------------------------------------------------------------- append
-int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames, const void* k,
-                 const void* v, uint32_t flags, void* cuda_stream) {
+// Append on `exec`; when `join` is another stream, `join` waits for the append and the completion that sessions and
+// freed pages remember is recorded on `join` (after everything enqueued there so far, e.g. the attention of the step).
+static int append_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames, const void* k,
+                       const void* v, uint32_t flags, cudaStream_t stream, cudaStream_t join) {
   if (pool == nullptr) return TS_ERR_INVALID;
   int rc = check_batch(pool, layer, n, sids, chunk_frames);
   if (rc != TS_OK) return rc;
@@ -701,7 +708,6 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, c
   if (k == nullptr || v == nullptr || (((uintptr_t)k | (uintptr_t)v) & 15) != 0) return TS_ERR_INVALID;
   if ((flags & ~(uint32_t)TS_COMMIT) != 0) return TS_ERR_INVALID;
   const ts_pool_config& c = pool->cfg;
-  cudaStream_t stream = (cudaStream_t)cuda_stream;
   TS_CUDA(cudaSetDevice(c.device));
   const int T = c.frame_tokens, B = c.page_tokens, W = c.window_frames;
 
@@ -779,7 +785,11 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, c
   ++pool->launches;
   TS_CUDA(cudaEventRecord(st->ev, stream));
   st->in_flight = true;
-  const uint64_t seq = pool->tl_compute.record(stream);
+  if (join != stream) {
+    TS_CUDA(cudaEventRecord(pool->ev_join, stream));
+    TS_CUDA(cudaStreamWaitEvent(join, pool->ev_join, 0));
+  }
+  const uint64_t seq = pool->tl_compute.record(join);
 
   for (int b = 0; b < n; ++b) {
     Session& s = pool->sess[sids[b]];
@@ -801,6 +811,46 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, c
     }
   }
   return TS_OK;
+}
+
+int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames, const void* k,
+                 const void* v, uint32_t flags, void* cuda_stream) {
+  return append_impl(pool, layer, n, sids, chunk_frames, k, v, flags, (cudaStream_t)cuda_stream, (cudaStream_t)cuda_stream);
+}
+
+// --------------------------------------------------------------------------------------------- fused device step
+int ts_chunk_step(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames, const void* q,
+                  const void* k, const void* v, void* out, float* lse, float scale, uint32_t flags, void* cuda_stream) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  int rc = check_batch(pool, layer, n, sids, chunk_frames);
+  if (rc != TS_OK) return rc;
+  if (n == 0) return TS_OK;
+  if (k == nullptr || v == nullptr || (((uintptr_t)k | (uintptr_t)v) & 15) != 0) return TS_ERR_INVALID;
+  if ((flags & ~(uint32_t)TS_COMMIT) != 0) return TS_ERR_INVALID;
+  {   // page demand of the append, before anything is enqueued (all-or-nothing)
+    const int T = pool->cfg.frame_tokens, B = pool->cfg.page_tokens;
+    int64_t need_total = 0;
+    for (int b = 0; b < n; ++b) {
+      const Session& s = pool->sess[sids[b]];
+      const int64_t end = (int64_t)s.o + (int64_t)s.P * T + (int64_t)chunk_frames[b] * T;
+      need_total += std::max<int64_t>(0, (end + B - 1) / B - (int64_t)s.pt.size());
+    }
+    if (need_total > (int64_t)pool->free_q.size()) return TS_ERR_NO_PAGES;
+  }
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  TS_CUDA(cudaSetDevice(pool->cfg.device));
+  if (pool->aux_s == nullptr) {
+    TS_CUDA(cudaStreamCreateWithFlags(&pool->aux_s, cudaStreamNonBlocking));
+    TS_CUDA(cudaEventCreateWithFlags(&pool->ev_fork, cudaEventDisableTiming));
+    TS_CUDA(cudaEventCreateWithFlags(&pool->ev_join, cudaEventDisableTiming));
+  }
+  // The append writes slots [L, L+C) that this step's attention does not read (R5), and it is HBM-bound while the
+  // attention is tensor-bound: it runs on a second stream under the attention kernel and joins `cuda_stream` after it.
+  TS_CUDA(cudaEventRecord(pool->ev_fork, stream));
+  TS_CUDA(cudaStreamWaitEvent(pool->aux_s, pool->ev_fork, 0));
+  rc = ts_chunk_attention(pool, layer, n, sids, chunk_frames, q, k, v, out, lse, scale, cuda_stream);
+  if (rc != TS_OK) return rc;
+  return append_impl(pool, layer, n, sids, chunk_frames, k, v, flags, pool->aux_s, stream);
 }
 
 // --------------------------------------------------------------------------------------------- gather

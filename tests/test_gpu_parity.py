@@ -583,3 +583,36 @@ def test_cluster_pairing_shapes(n_heads, priors, chunks):
     q, k, v = (draw(rng, total, shape) for _ in range(3))
     dp.attention(0, sids, [min(c, 2) for c in chunks], *(x[:sum(min(c, 2) for c in chunks) * T] for x in (q, k, v)),
                  scale_of(shape))
+
+
+# ---- ts_chunk_step: attention + append as one call, the append running under the attention on a pool stream --------
+def test_chunk_step_fused_equals_sequence():
+    from paper_2606_19271_b200 import TS_COMMIT
+    shape = shape_of(n_heads=3, head_dim=128, frame_tokens=203, window_frames=5, page_tokens=64, n_pages=128)
+    rng = np.random.default_rng(21)
+    dp = DualPool(shape, rng.permutation(shape.n_pages))
+    T = shape.frame_tokens
+    sids = [dp.open(), dp.open(), dp.open()]
+    cf = [2, 1, 3]
+    n_tok = sum(cf) * T
+    for step in range(4):                      # the window of the 3-frame session fills and rolls at step 2
+        q, k, v = (draw(rng, n_tok, shape) for _ in range(3))
+        o_ref, _ = oracle.chunk_attention(dp.o, 0, sids, cf, q, k, v, scale_of(shape))
+        dq, dk, dv = bits_to_dev(q), bits_to_dev(k), bits_to_dev(v)
+        out = torch.full_like(dq, float("nan"))
+        dp.g.ts_chunk_step(0, sids, cf, dq, dk, dv, out, None, float(scale_of(shape)), TS_COMMIT)
+        dp.o.append(0, sids, cf, k, v, commit=True)
+        torch.cuda.synchronize()
+        o_gpu = out.double().cpu().numpy()
+        assert np.abs(o_gpu - o_ref).max() <= 2e-2 and rel_l2(o_gpu, o_ref) <= 5e-3
+        dp.check_state(sids, kv=True)
+    # all-or-nothing: a step that cannot get its pages changes nothing and enqueues nothing
+    big = shape_of(n_heads=3, head_dim=128, frame_tokens=203, window_frames=0, page_tokens=64, n_pages=8)
+    dq2 = DualPool(big, None)
+    s0 = dq2.open()
+    q, k, v = (draw(rng, 3 * T, big) for _ in range(3))
+    import paper_2606_19271_b200 as tc
+    with pytest.raises(tc.TurboChunkError) as e:
+        dq2.g.ts_chunk_step(0, [s0], [3], bits_to_dev(q), bits_to_dev(k), bits_to_dev(v), torch.empty(3 * T, 3, 128, dtype=torch.bfloat16, device="cuda"), None, 0.1, TS_COMMIT)
+    assert e.value.code == tc.TS_ERR_NO_PAGES
+    dq2.check_state([s0])
