@@ -43,7 +43,8 @@ struct Cfg {
   static constexpr int kSmemQ = 2 * kTileBytes;
   static constexpr int kSmemKV = kSlots * kTileBytes;
   static constexpr int kNumBars = 2 * kSlots + 2 + 10;
-  static constexpr int kSmemBytes = 1024 + kSmemQ + kSmemKV + kNumBars * 8 + 16;
+  static constexpr int kXchgBytes = 2 * 128 * 2 * 4;    // (m, l) of a row from each softmax warpgroup (lone-tile merge)
+  static constexpr int kSmemBytes = kSmemQ + kSmemKV + kXchgBytes + kNumBars * 8 + 16;
 };
 
 struct ItemGeom {
@@ -51,6 +52,7 @@ struct ItemGeom {
   int x_begin, x_end, t0, n_prior, n_chunk, n_kv;
   int n_pipe;   // KV tiles flowing through the smem ring for this item (>= n_kv: the cluster partner may see more)
   bool mc;      // K/V tiles are loaded half by this CTA, half by the cluster partner, multicast to both
+  bool split;   // lone query tile: its KV tiles alternate between the two TMEM tile slots (even / odd), merged at the end
 };
 
 __device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int idx) {
@@ -87,17 +89,18 @@ __device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int idx) {
     g.n_chunk = (kv_hi + 127) >> 7;
     g.n_kv = g.n_prior + g.n_chunk;
   }
+  g.split = (g.n_q == 1) && (g.n_kv >= 2);
   return g;
 }
 
 template <int D>
 __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __grid_constant__ AttnParams p) {
   using C = Cfg<D>;
-  extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  extern __shared__ __align__(1024) uint8_t smem[];   // swizzle-128B operands need 1024-byte alignment
   uint8_t* sQ = smem;
   uint8_t* sKV = smem + C::kSmemQ;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + C::kSmemKV);
+  float2* xchg = reinterpret_cast<float2*>(sKV + C::kSmemKV);   // [warpgroup][row]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sKV + C::kSmemKV + C::kXchgBytes);
   uint64_t* kv_full = bars;
   uint64_t* kv_empty = bars + C::kSlots;
   uint64_t* q_full = bars + 2 * C::kSlots;
@@ -112,6 +115,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
   const int lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
+    if (smem_u32(smem) & 1023u) __trap();
     for (int i = 0; i < C::kSlots; ++i) {
       mbar_init(&kv_full[i], 1);
       mbar_init(&kv_empty[i], 2);   // released by the MMA warps of both CTAs of the cluster
@@ -123,7 +127,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
       mbar_init(&p_half[2 * i], 128);
       mbar_init(&p_half[2 * i + 1], 128);
       mbar_init(&o_done[i], 1);
-      mbar_init(&o_free[i], 128);
+      mbar_init(&o_free[i], 256);   // two arrivals per thread of the tile's warpgroup, or one from each of both
     }
     fence_mbar_init();
     tma_prefetch_desc(&p.map_k);
@@ -208,8 +212,9 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
       constexpr uint32_t idesc_pv = make_idesc_bf16(128, D, 0, 1);
       const uint32_t sQ_addr = smem_u32(sQ);
       const uint32_t sKV_addr = smem_u32(sKV);
-      auto issue_s = [&](int i, uint32_t slot) {
-        const uint32_t a = sQ_addr + i * C::kTileBytes;
+      // S of TMEM tile slot `i` = (query tile `qi` in smem) x (K tile in ring slot `slot`)^T
+      auto issue_s_q = [&](int qi, int i, uint32_t slot) {
+        const uint32_t a = sQ_addr + qi * C::kTileBytes;
         const uint32_t b = sKV_addr + slot * C::kTileBytes;
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
@@ -218,6 +223,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
                  idesc_s, kk > 0);
         }
       };
+      auto issue_s = [&](int i, uint32_t slot) { issue_s_q(i, i, slot); };
       // half h of O_i += P_i V: the 16-key steps 4h .. 4h+3 (keys [64h, 64h+64))
       auto issue_pv_half = [&](int i, uint32_t slot, int h, bool acc) {
         const uint32_t b = sKV_addr + slot * C::kTileBytes;
@@ -237,6 +243,50 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
         // when the two work on unrelated items: a slot is refilled (possibly by the partner's multicast) only after
         // both CTAs are done with their tile at that ring position
         auto release = [&](uint32_t slot) { mma_commit_mc(&kv_empty[slot], 3); };
+        if (g.split) {
+          // lone query tile: K/V tile j goes to TMEM tile slot j & 1, so two tiles are in flight as for a pair.
+          // Ring positions relative to the item: K_j at 2j, V_j at 2j + 1.
+          const uint32_t base = kv_it;
+          mbar_wait(q_full, q_cnt & 1);
+          ++q_cnt;
+          for (int i = 0; i < 2; ++i) {
+            const uint32_t it = base + 2 * i, slot = it % C::kSlots, ph = (it / C::kSlots) & 1;
+            mbar_wait(&kv_full[slot], ph);
+            tc_fence_after();
+            issue_s_q(0, i, slot);
+            mma_commit(&s_full[i]);
+            release(slot);
+          }
+          if (g.n_kv == 2) mma_commit(q_empty);
+          for (int j = 0; j < g.n_kv; ++j) {
+            const int i = j & 1;
+            const uint32_t it_v = base + 2 * j + 1, slot_v = it_v % C::kSlots, ph_v = (it_v / C::kSlots) & 1;
+            const uint32_t par = cnt_p[i] & 1;
+            ++cnt_p[i];
+            mbar_wait(&p_half[2 * i], par);
+            mbar_wait(&kv_full[slot_v], ph_v);
+            if (j < 2) mbar_wait(&o_free[i], (cnt_items[i] & 1) ^ 1);
+            tc_fence_after();
+            issue_pv_half(i, slot_v, 0, j >= 2);
+            mbar_wait(&p_half[2 * i + 1], par);
+            tc_fence_after();
+            issue_pv_half(i, slot_v, 1, true);
+            mma_commit(&o_done[i]);
+            release(slot_v);
+            if (j + 2 < g.n_kv) {
+              const uint32_t it_k = base + 2 * (j + 2), slot_k = it_k % C::kSlots, ph_k = (it_k / C::kSlots) & 1;
+              mbar_wait(&kv_full[slot_k], ph_k);
+              tc_fence_after();
+              issue_s_q(0, i, slot_k);
+              mma_commit(&s_full[i]);
+              release(slot_k);
+              if (j + 3 == g.n_kv) mma_commit(q_empty);
+            }
+          }
+          kv_it = base + 2 * g.n_kv;
+          ++cnt_items[0];
+          ++cnt_items[1];
+        } else {
         if (g.n_q > 0) {
           mbar_wait(q_full, q_cnt & 1);
           ++q_cnt;
@@ -289,6 +339,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
           }
         }
         for (int i = 0; i < g.n_q; ++i) ++cnt_items[i];
+        }
         // K/V tiles only the cluster partner needs (it sees more chunk frames, or this CTA has no query rows)
         for (int e = 2 * g.n_kv; e < 2 * g.n_pipe; ++e) {
           const uint32_t slot = kv_it % C::kSlots, ph = (kv_it / C::kSlots) & 1;
@@ -309,16 +360,25 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
     const uint32_t taddr_o = tmem_base + lane_sel + 256 + wg * D;
     const float c = p.scale_log2;
     const float thr = kRescaleThresholdLog2 / c;
+    const uint32_t taddr_o_other = tmem_base + lane_sel + 256 + (wg ^ 1) * D;
     uint32_t cnt_s = 0, cnt_pv = 0;
+    uint32_t cnt_pv_other = 0;                            // PV groups committed so far on the OTHER tile slot
     for (int idx = it_begin; idx < it_end; ++idx) {
       const ItemGeom g = decode_item(p, idx);
-      if (wg >= g.n_q) continue;
-      const int first_row = g.r0 + 128 * wg;
+      if (!g.split && wg >= g.n_q) {
+        if (g.n_q == 1) cnt_pv_other += g.n_kv;           // warpgroup 1 sits out a lone tile that runs on slot 0 alone
+        continue;
+      }
+      // a split lone tile: both warpgroups work on the SAME 128 query rows, this one on KV tiles wg, wg+2, ...
+      const int j0 = g.split ? wg : 0, dj = g.split ? 2 : 1;
+      const int first_row = g.r0 + (g.split ? 0 : 128 * wg);
       const int row = first_row + row_in_tile;
       const int lim_row = min(g.C, (min(row, g.C - 1) / p.T + 1) * p.T);   // chunk keys visible to this row
       const int lim_min = min(g.C, (first_row / p.T + 1) * p.T);           // ... to the tile's first row
-      float m = -INFINITY, l = 0.f;
-      for (int j = 0; j < g.n_kv; ++j) {
+      // -1e30 rather than -inf: a split tile's first KV tile may hold no visible key for a row (all scores -inf);
+      // (-inf) - (-1e30) = -inf gives p = 0 where (-inf) - (-inf) would give NaN
+      float m = -1e30f, l = 0.f;
+      for (int j = j0; j < g.n_kv; j += dj) {
         mbar_wait(&s_full[wg], cnt_s & 1);
         ++cnt_s;
         tc_fence_after();
@@ -357,8 +417,8 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
         mx0 = max3(mx0, __uint_as_float(s[124]), __uint_as_float(s[125]));
         mx1 = max3(mx1, __uint_as_float(s[126]), __uint_as_float(s[127]));
         const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-        if (j == 0) {
-          m = mx;   // the first tile of an item always holds a visible key for every row
+        if (j == j0) {
+          m = fmaxf(mx, m);   // first tile of the row: nothing accumulated yet, no rescale
         } else {
           const bool need = mx > m + thr;
           if (__any_sync(0xffffffffu, need)) {
@@ -412,33 +472,78 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
         l += (l0 + l1) + (l2 + l3);
         ++cnt_pv;
       }
-      // ---- epilogue: O / l -> bf16 -> global
-      mbar_wait(&o_done[wg], (cnt_pv - 1) & 1);
-      tc_fence_after();
-      const float inv_l = 1.0f / l;
       const bool store = row < g.C;
       uint16_t* orow = p.out + ((size_t)(g.q_off + row) * p.H + g.head) * D;
+      if (!g.split) {
+        // ---- epilogue: O / l -> bf16 -> global
+        if (g.n_q == 2) cnt_pv_other += g.n_kv;
+        mbar_wait(&o_done[wg], (cnt_pv - 1) & 1);
+        tc_fence_after();
+        const float inv_l = 1.0f / l;
 #pragma unroll
-      for (int cc = 0; cc < D; cc += 32) {
-        uint32_t o[32];
-        tmem_ld32(taddr_o + cc, o);
-        tmem_ld_wait();
-        if (store) {
+        for (int cc = 0; cc < D; cc += 32) {
+          uint32_t o[32];
+          tmem_ld32(taddr_o + cc, o);
+          tmem_ld_wait();
+          if (store) {
 #pragma unroll
-          for (int k = 0; k < 32; k += 8) {
-            uint4 v;
-            v.x = pack_bf16x2(__uint_as_float(o[k + 0]) * inv_l, __uint_as_float(o[k + 1]) * inv_l);
-            v.y = pack_bf16x2(__uint_as_float(o[k + 2]) * inv_l, __uint_as_float(o[k + 3]) * inv_l);
-            v.z = pack_bf16x2(__uint_as_float(o[k + 4]) * inv_l, __uint_as_float(o[k + 5]) * inv_l);
-            v.w = pack_bf16x2(__uint_as_float(o[k + 6]) * inv_l, __uint_as_float(o[k + 7]) * inv_l);
-            *reinterpret_cast<uint4*>(orow + cc + k) = v;
+            for (int k = 0; k < 32; k += 8) {
+              uint4 v;
+              v.x = pack_bf16x2(__uint_as_float(o[k + 0]) * inv_l, __uint_as_float(o[k + 1]) * inv_l);
+              v.y = pack_bf16x2(__uint_as_float(o[k + 2]) * inv_l, __uint_as_float(o[k + 3]) * inv_l);
+              v.z = pack_bf16x2(__uint_as_float(o[k + 4]) * inv_l, __uint_as_float(o[k + 5]) * inv_l);
+              v.w = pack_bf16x2(__uint_as_float(o[k + 6]) * inv_l, __uint_as_float(o[k + 7]) * inv_l);
+              *reinterpret_cast<uint4*>(orow + cc + k) = v;
+            }
           }
         }
+        tc_fence_before();
+        mbar_arrive_n(&o_free[wg], 2);
+        if (p.lse != nullptr && store)
+          p.lse[(size_t)(g.q_off + row) * p.H + g.head] = (m * c + log2f(l)) * 0.6931471805599453f;
+      } else {
+        // ---- epilogue of a split lone tile: merge the two partial softmax states of every row.  The two threads of
+        //      a row swap (m, l) through smem; each then reads BOTH partial O rows from TMEM (same lanes) for its half
+        //      of the D columns:  O = (a_own O_own + a_oth O_oth) / (a_own l_own + a_oth l_oth),  a = 2^((m - m_tot) c)
+        cnt_pv_other += (uint32_t)((g.n_kv - (wg ^ 1) + 1) >> 1);
+        const int bar_id = 1 + (warp & 3);
+        xchg[wg * 128 + row_in_tile] = make_float2(m, l);
+        named_bar_sync(bar_id, 64);
+        const float2 oth = xchg[(wg ^ 1) * 128 + row_in_tile];
+        named_bar_sync(bar_id, 64);                       // both reads are done before the next split item writes
+        const float m_tot = fmaxf(m, oth.x);
+        const float a_own = ex2_approx((m - m_tot) * c), a_oth = ex2_approx((oth.x - m_tot) * c);
+        const float l_tot = a_own * l + a_oth * oth.y;
+        const float inv_l = 1.0f / l_tot;
+        const float w_own = a_own * inv_l, w_oth = a_oth * inv_l;
+        mbar_wait(&o_done[wg], (cnt_pv - 1) & 1);
+        mbar_wait(&o_done[wg ^ 1], (cnt_pv_other - 1) & 1);
+        tc_fence_after();
+        const int col0 = wg * (D / 2);
+#pragma unroll
+        for (int cc = 0; cc < D / 2; cc += 32) {
+          uint32_t o[32], q[32];
+          tmem_ld32(taddr_o + col0 + cc, o);
+          tmem_ld32(taddr_o_other + col0 + cc, q);
+          tmem_ld_wait();
+          if (store) {
+#pragma unroll
+            for (int k = 0; k < 32; k += 8) {
+              uint32_t r[4];
+#pragma unroll
+              for (int t = 0; t < 4; ++t)
+                r[t] = pack_bf16x2(__uint_as_float(o[k + 2 * t]) * w_own + __uint_as_float(q[k + 2 * t]) * w_oth,
+                                   __uint_as_float(o[k + 2 * t + 1]) * w_own + __uint_as_float(q[k + 2 * t + 1]) * w_oth);
+              *reinterpret_cast<uint4*>(orow + col0 + cc + k) = make_uint4(r[0], r[1], r[2], r[3]);
+            }
+          }
+        }
+        tc_fence_before();
+        mbar_arrive(&o_free[0]);
+        mbar_arrive(&o_free[1]);
+        if (p.lse != nullptr && store && wg == 0)
+          p.lse[(size_t)(g.q_off + row) * p.H + g.head] = (m_tot * c + log2f(l_tot)) * 0.6931471805599453f;
       }
-      tc_fence_before();
-      mbar_arrive(&o_free[wg]);
-      if (p.lse != nullptr && store)
-        p.lse[(size_t)(g.q_off + row) * p.H + g.head] = (m * c + log2f(l)) * 0.6931471805599453f;
     }
   }
 

@@ -536,8 +536,8 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
         item_geometry(c, C, d.x_begin, d.x_end, qp, &n_q, &n_kv);
         // time model in twentieths of a two-tile KV step, fitted to per-CTA cycle counts on configs[2]
         // (3184 clk per step + 14.7 k clk per item): 4.5 steps per item for the Q load, pipeline fill and epilogue.
-        // A lone query tile has no ping-pong partner to hide its S -> softmax -> PV chain behind: ~0.95 of a pair step.
-        const int cost = (n_q == 2 ? 20 : 19) * n_kv + 90;
+        // A lone query tile alternates its KV tiles between the two TMEM tile slots (half the steps, plus the merge).
+        const int cost = n_q == 2 ? 20 * n_kv + 90 : (n_kv >= 2 ? 10 * n_kv + 110 : 19 * n_kv + 90);
         for (int h = 0; h < H; ++h) cands.push_back({cost, b, h, qp, n_kv});
       }
       q_off += C;
