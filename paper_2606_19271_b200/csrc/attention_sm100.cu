@@ -61,7 +61,7 @@ __device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int idx) {
   ItemGeom g;
   g.sess = w.sess;
   g.head = w.head;
-  g.r0 = w.q_pair * 256;
+  g.r0 = w.q_tile * 128;
   g.C = s.C;
   g.q_off = s.q_off;
   g.pt_off = s.pt_off;
@@ -77,14 +77,14 @@ __device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int idx) {
     g.t0 = 0;
     g.n_prior = 0;
   }
-  if (w.q_pair < 0) {   // no query rows: only the loader and the slot releases run
+  if (w.q_tile < 0) {   // no query rows: only the loader and the slot releases run
     g.r0 = 0;
     g.n_q = 0;
     g.n_chunk = 0;
     g.n_kv = 0;
   } else {
-    g.n_q = (g.r0 + 128 < s.C) ? 2 : 1;
-    const int last_row = min(s.C, g.r0 + 256) - 1;
+    g.n_q = (!(w.pipe & 0x40000000u) && g.r0 + 128 < s.C) ? 2 : 1;
+    const int last_row = min(s.C, g.r0 + 128 * g.n_q) - 1;
     const int kv_hi = min(s.C, (last_row / p.T + 1) * p.T);   // chunk keys visible to the item's last row
     g.n_chunk = (kv_hi + 127) >> 7;
     g.n_kv = g.n_prior + g.n_chunk;

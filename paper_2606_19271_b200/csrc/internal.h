@@ -23,14 +23,15 @@ struct SessDesc {      // one per session of the batch
 };
 static_assert(sizeof(SessDesc) == 32, "SessDesc layout");
 
-struct WorkItem {      // one (session, head, pair of 128-row query tiles) for one CTA of a 2-CTA cluster
+struct WorkItem {      // one (session, head, one or two 128-row query tiles) for one CTA of a 2-CTA cluster
   int32_t sess;        // index into the batch
   int32_t head;
-  int32_t q_pair;      // query rows [256*q_pair, 256*q_pair + 256) of the session's chunk; -1: no query rows (the CTA
+  int32_t q_tile;      // first query tile: rows [128*q_tile, ...) of the session's chunk; -1: no query rows (the CTA
                        // only loads its half of the partner's K/V tiles)
   uint32_t pipe;       // bits 0-23: KV tiles that flow through this CTA's smem ring for the item (>= the item's own
                        // KV tiles); bit 31: the two CTAs of the cluster work on the same (session, head) and each
-                       // loads half of every K/V tile, multicast to both
+                       // loads half of every K/V tile, multicast to both; bit 30: one query tile only, also when
+                       // the chunk has rows left for a second one
 };
 static_assert(sizeof(WorkItem) == 16, "WorkItem layout");
 

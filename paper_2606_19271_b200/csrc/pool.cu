@@ -237,10 +237,11 @@ struct ScheduleLayout {
   int n_items, grid;
 };
 
-static void item_geometry(const ts_pool_config& c, int C, int x_begin, int x_end, int q_pair, int* n_q, int* n_kv) {
-  const int r0 = q_pair * 256;
-  *n_q = (r0 + 128 < C) ? 2 : 1;
-  const int last_row = std::min(C, r0 + 256) - 1;
+static void item_geometry(const ts_pool_config& c, int C, int x_begin, int x_end, int q_tile, int max_tiles, int* n_q,
+                          int* n_kv) {
+  const int r0 = q_tile * 128;
+  *n_q = (max_tiles >= 2 && r0 + 128 < C) ? 2 : 1;
+  const int last_row = std::min(C, r0 + 128 * *n_q) - 1;
   const int kv_hi = std::min(C, (last_row / c.frame_tokens + 1) * c.frame_tokens);
   const int n_chunk = (kv_hi + 127) / 128;
   const int n_prior = x_end > x_begin ? ((x_end - 1) / 128 - x_begin / 128 + 1) : 0;
@@ -511,10 +512,6 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
     std::vector<WorkItem>& items = pool->sched_items;
     sd.assign(n, SessDesc());
     pt.clear();
-    struct Cand {
-      int cost, sess, head, q_pair, n_kv;
-    };
-    std::vector<Cand> cands;
     int q_off = 0;
     for (int b = 0; b < n; ++b) {
       const Session& s = pool->sess[sids[b]];
@@ -530,106 +527,129 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
       d.n_pt = (int32_t)s.pt.size();
       d.pad0 = d.pad1 = 0;
       pt.insert(pt.end(), s.pt.begin(), s.pt.end());
-      const int n_pairs = (C + 255) / 256;
-      for (int qp = 0; qp < n_pairs; ++qp) {
-        int n_q, n_kv;
-        item_geometry(c, C, d.x_begin, d.x_end, qp, &n_q, &n_kv);
-        // time model in twentieths of a two-tile KV step, fitted to per-CTA cycle counts on configs[2]
-        // (3184 clk per step + 14.7 k clk per item): 4.5 steps per item for the Q load, pipeline fill and epilogue.
-        // A lone query tile alternates its KV tiles between the two TMEM tile slots (half the steps, plus the merge).
-        const int cost = n_q == 2 ? 20 * n_kv + 90 : (n_kv >= 2 ? 10 * n_kv + 110 : 19 * n_kv + 90);
-        for (int h = 0; h < H; ++h) cands.push_back({cost, b, h, qp, n_kv});
-      }
       q_off += C;
     }
-    // ---- cluster items.  The q-pair items of one (session, head) stream read the same K/V pages: two of them at a
-    // time go to the two CTAs of a cluster, which then load half of every K/V tile each and multicast it to both
-    // (mc).  A stream's odd item out is paired with another stream's (or with nothing): those two share a cluster
-    // without sharing loads.  Both CTAs cycle max(n_kv) tiles through their smem rings so that they stay on the same
-    // ring position.
+    // Work items come in two granularities: pairs of 128-row query tiles (one K/V tile feeds 256 rows), or single
+    // tiles whose KV tiles alternate between the two TMEM tile slots (half as long, same MMA work per step, twice the
+    // K/V traffic per FLOP).  Pairs are the default; single tiles are taken when the batch is so small that pairs
+    // leave clusters idle in the last wave (1-2 sessions), judged by the modelled makespan of both schedules.
+    struct Cand {
+      int cost, sess, head, q_tile, n_kv;
+      bool single;
+    };
     struct CItem {
       int cost;
       int64_t stream_cost;
       int stream;
-      Cand a, b;       // b.q_pair < 0: no second item
+      Cand a, b;       // b.q_tile < 0: no second item
       bool mc;
     };
-    std::vector<int64_t> stream_cost((size_t)n * H, 0);
-    for (const Cand& x : cands) stream_cost[(size_t)x.sess * H + x.head] += x.cost;
-    // within a stream: by KV length (longest first), two-tile items before a lone tile
-    std::stable_sort(cands.begin(), cands.end(), [&](const Cand& x, const Cand& y) {
-      const size_t sx = (size_t)x.sess * H + x.head, sy = (size_t)y.sess * H + y.head;
-      if (sx != sy) return sx < sy;
-      if (x.n_kv != y.n_kv) return x.n_kv > y.n_kv;
-      return x.cost > y.cost;
-    });
-    std::vector<CItem> citems;
-    std::vector<Cand> odd;
-    for (size_t i = 0; i < cands.size();) {
-      size_t e = i;
-      while (e < cands.size() && cands[e].sess == cands[i].sess && cands[e].head == cands[i].head) ++e;
-      const int stream = cands[i].sess * H + cands[i].head;
-      // pair items of EQUAL KV length first (neither CTA then waits for tiles only its partner needs); what is left
-      // over (at most one item per length) is paired in length order, and the stream's last odd item goes to `odd`
-      std::vector<Cand> rest;
-      while (i < e) {
-        if (i + 1 < e && cands[i].n_kv == cands[i + 1].n_kv) {
-          citems.push_back({std::max(cands[i].cost, cands[i + 1].cost), stream_cost[stream], stream, cands[i], cands[i + 1], true});
-          i += 2;
-        } else {
-          rest.push_back(cands[i++]);
+    struct Plan {
+      std::vector<CItem> citems;
+      std::vector<std::vector<int>> per_cluster;
+      int64_t makespan = 0;
+    };
+    auto make_plan = [&](int tiles_per_item) {
+      Plan plan;
+      std::vector<Cand> cands;
+      for (int b = 0; b < n; ++b) {
+        const SessDesc& d = sd[b];
+        const int n_tiles = (d.C + 127) / 128;
+        for (int t0 = 0; t0 < n_tiles; t0 += tiles_per_item) {
+          int n_q, n_kv;
+          item_geometry(c, d.C, d.x_begin, d.x_end, t0, tiles_per_item, &n_q, &n_kv);
+          // time model in twentieths of a two-tile KV step, fitted to per-CTA cycle counts on configs[2]
+          // (3184 clk per step + 14.7 k clk per item): 4.5 steps per item for the Q load, pipeline fill and epilogue.
+          // A lone query tile alternates its KV tiles between the two TMEM tile slots (half the steps, plus the merge).
+          const int cost = n_q == 2 ? 20 * n_kv + 90 : (n_kv >= 2 ? 10 * n_kv + 110 : 19 * n_kv + 90);
+          for (int h = 0; h < H; ++h) cands.push_back({cost, b, h, t0, n_kv, tiles_per_item == 1});
         }
       }
-      size_t r = 0;
-      for (; r + 1 < rest.size(); r += 2)
-        citems.push_back({std::max(rest[r].cost, rest[r + 1].cost), stream_cost[stream], stream, rest[r], rest[r + 1], true});
-      if (r < rest.size()) odd.push_back(rest[r]);
-    }
-    std::stable_sort(odd.begin(), odd.end(), [](const Cand& x, const Cand& y) { return x.cost > y.cost; });
-    for (size_t i = 0; i < odd.size(); i += 2) {
-      Cand none = odd[i];
-      none.q_pair = -1;
-      none.n_kv = 0;
-      none.cost = 0;
-      const Cand& second = (i + 1 < odd.size()) ? odd[i + 1] : none;
-      const int stream = odd[i].sess * H + odd[i].head;
-      citems.push_back({std::max(odd[i].cost, second.cost), stream_cost[stream], stream, odd[i], second, false});
-    }
-    // List scheduling in stream order, heaviest streams first (LPT at stream granularity, so that the tail of the
-    // schedule is made of short items): a stream's items are dealt out back to back, each to the least-loaded
-    // cluster, and run at the same time - the stream's K/V then comes from DRAM once and from L2 afterwards.
-    std::stable_sort(citems.begin(), citems.end(), [](const CItem& x, const CItem& y) {
-      if (x.stream_cost != y.stream_cost) return x.stream_cost > y.stream_cost;
-      if (x.stream != y.stream) return x.stream < y.stream;
-      return x.cost > y.cost;
-    });
-    const int n_clusters = std::min(grid_max / 2, (int)citems.size());
-    const int grid = 2 * n_clusters;
-    std::vector<std::vector<int>> per_cluster(n_clusters);
-    {
+      // ---- cluster items.  The items of one (session, head) stream read the same K/V pages: two of them at a time
+      // go to the two CTAs of a cluster, which then load half of every K/V tile each and multicast it to both (mc).
+      // A stream's odd item out is paired with another stream's (or with nothing): those two share a cluster without
+      // sharing loads.  Both CTAs cycle max(n_kv) tiles through their smem rings to stay on the same ring position.
+      std::vector<int64_t> stream_cost((size_t)n * H, 0);
+      for (const Cand& x : cands) stream_cost[(size_t)x.sess * H + x.head] += x.cost;
+      // within a stream: by KV length (longest first), two-tile items before a lone tile
+      std::stable_sort(cands.begin(), cands.end(), [&](const Cand& x, const Cand& y) {
+        const size_t sx = (size_t)x.sess * H + x.head, sy = (size_t)y.sess * H + y.head;
+        if (sx != sy) return sx < sy;
+        if (x.n_kv != y.n_kv) return x.n_kv > y.n_kv;
+        return x.cost > y.cost;
+      });
+      std::vector<CItem>& citems = plan.citems;
+      std::vector<Cand> odd;
+      for (size_t i = 0; i < cands.size();) {
+        size_t e = i;
+        while (e < cands.size() && cands[e].sess == cands[i].sess && cands[e].head == cands[i].head) ++e;
+        const int stream = cands[i].sess * H + cands[i].head;
+        // pair items of EQUAL KV length first (neither CTA then waits for tiles only its partner needs); what is left
+        // over (at most one item per length) is paired in length order, and the stream's last odd item goes to `odd`
+        std::vector<Cand> rest;
+        while (i < e) {
+          if (i + 1 < e && cands[i].n_kv == cands[i + 1].n_kv) {
+            citems.push_back({std::max(cands[i].cost, cands[i + 1].cost), stream_cost[stream], stream, cands[i], cands[i + 1], true});
+            i += 2;
+          } else {
+            rest.push_back(cands[i++]);
+          }
+        }
+        size_t r = 0;
+        for (; r + 1 < rest.size(); r += 2)
+          citems.push_back({std::max(rest[r].cost, rest[r + 1].cost), stream_cost[stream], stream, rest[r], rest[r + 1], true});
+        if (r < rest.size()) odd.push_back(rest[r]);
+      }
+      std::stable_sort(odd.begin(), odd.end(), [](const Cand& x, const Cand& y) { return x.cost > y.cost; });
+      for (size_t i = 0; i < odd.size(); i += 2) {
+        Cand none = odd[i];
+        none.q_tile = -1;
+        none.n_kv = 0;
+        none.cost = 0;
+        const Cand& second = (i + 1 < odd.size()) ? odd[i + 1] : none;
+        const int stream = odd[i].sess * H + odd[i].head;
+        citems.push_back({std::max(odd[i].cost, second.cost), stream_cost[stream], stream, odd[i], second, false});
+      }
+      // List scheduling in stream order, heaviest streams first (LPT at stream granularity, so that the tail of the
+      // schedule is made of short items): a stream's items are dealt out back to back, each to the least-loaded
+      // cluster, and run at the same time - the stream's K/V then comes from DRAM once and from L2 afterwards.
+      std::stable_sort(citems.begin(), citems.end(), [](const CItem& x, const CItem& y) {
+        if (x.stream_cost != y.stream_cost) return x.stream_cost > y.stream_cost;
+        if (x.stream != y.stream) return x.stream < y.stream;
+        return x.cost > y.cost;
+      });
+      const int n_clusters = std::min(grid_max / 2, (int)citems.size());
+      plan.per_cluster.assign(n_clusters, std::vector<int>());
       typedef std::pair<int64_t, int> Load;   // (load, cluster)
       std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
       for (int i = 0; i < n_clusters; ++i) heap.push({0, i});
       for (int i = 0; i < (int)citems.size(); ++i) {
         Load top = heap.top();
         heap.pop();
-        per_cluster[top.second].push_back(i);
+        plan.per_cluster[top.second].push_back(i);
         heap.push({top.first + citems[i].cost, top.second});
+        plan.makespan = std::max(plan.makespan, top.first + citems[i].cost);
       }
+      return plan;
+    };
+    Plan plan = make_plan(2);
+    if (n * H * 2 <= grid_max) {               // small batch: fewer than two streams per cluster
+      Plan fine = make_plan(1);
+      if (fine.makespan * 108 < plan.makespan * 100) plan = std::move(fine);   // single tiles cost ~8 % more per FLOP
     }
-
+    const int grid = 2 * (int)plan.per_cluster.size();
     cta_begin.assign(grid + 1, 0);
     items.clear();
     for (int ci = 0; ci < grid; ++ci) {
       cta_begin[ci] = (int32_t)items.size();
-      for (int i : per_cluster[ci >> 1]) {
-        const CItem& it = citems[i];
+      for (int i : plan.per_cluster[ci >> 1]) {
+        const CItem& it = plan.citems[i];
         const Cand& x = (ci & 1) ? it.b : it.a;
         WorkItem wi;
         wi.sess = x.sess;
         wi.head = x.head;
-        wi.q_pair = x.q_pair;
-        wi.pipe = (uint32_t)std::max(it.a.n_kv, it.b.n_kv) | (it.mc ? 0x80000000u : 0u);
+        wi.q_tile = x.q_tile;
+        wi.pipe = (uint32_t)std::max(it.a.n_kv, it.b.n_kv) | (it.mc ? 0x80000000u : 0u) | (x.single ? 0x40000000u : 0u);
         items.push_back(wi);
       }
     }
