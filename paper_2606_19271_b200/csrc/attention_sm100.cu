@@ -235,8 +235,8 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
         }
       };
       uint32_t kv_it = 0, q_cnt = 0;
-      uint32_t cnt_p[2] = {0, 0};
-      uint32_t cnt_items[2] = {0, 0};
+      // per tile slot: P hand-offs and items so far (scalars with selects: a runtime-indexed array would live in local memory)
+      uint32_t cnt_p0 = 0, cnt_p1 = 0, cnt_it0 = 0, cnt_it1 = 0;
       for (int idx = it_begin; idx < it_end; ++idx) {
         const ItemGeom g = decode_item(p, idx);
         // hand a K/V slot back once every MMA issued so far has read it - always to BOTH CTAs of the cluster, also
@@ -261,11 +261,12 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
           for (int j = 0; j < g.n_kv; ++j) {
             const int i = j & 1;
             const uint32_t it_v = base + 2 * j + 1, slot_v = it_v % C::kSlots, ph_v = (it_v / C::kSlots) & 1;
-            const uint32_t par = cnt_p[i] & 1;
-            ++cnt_p[i];
+            const uint32_t par = (i ? cnt_p1 : cnt_p0) & 1;
+            cnt_p0 += (i == 0);
+            cnt_p1 += (i != 0);
             mbar_wait(&p_half[2 * i], par);
             mbar_wait(&kv_full[slot_v], ph_v);
-            if (j < 2) mbar_wait(&o_free[i], (cnt_items[i] & 1) ^ 1);
+            if (j < 2) mbar_wait(&o_free[i], ((i ? cnt_it1 : cnt_it0) & 1) ^ 1);
             tc_fence_after();
             issue_pv_half(i, slot_v, 0, j >= 2);
             mbar_wait(&p_half[2 * i + 1], par);
@@ -284,8 +285,8 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
             }
           }
           kv_it = base + 2 * g.n_kv;
-          ++cnt_items[0];
-          ++cnt_items[1];
+          ++cnt_it0;
+          ++cnt_it1;
         } else {
         if (g.n_q > 0) {
           mbar_wait(q_full, q_cnt & 1);
@@ -312,11 +313,12 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
             ++kv_it;
           }
           for (int i = 0; i < g.n_q; ++i) {
-            const uint32_t par = cnt_p[i] & 1;
-            ++cnt_p[i];
+            const uint32_t par = (i ? cnt_p1 : cnt_p0) & 1;
+            cnt_p0 += (i == 0);
+            cnt_p1 += (i != 0);
             mbar_wait(&p_half[2 * i], par);
             if (i == 0) mbar_wait(&kv_full[slot_v], ph_v);
-            if (j == 0) mbar_wait(&o_free[i], (cnt_items[i] & 1) ^ 1);
+            if (j == 0) mbar_wait(&o_free[i], ((i ? cnt_it1 : cnt_it0) & 1) ^ 1);
             tc_fence_after();
             issue_pv_half(i, slot_v, 0, j > 0);
             mbar_wait(&p_half[2 * i + 1], par);
@@ -338,7 +340,8 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
             }
           }
         }
-        for (int i = 0; i < g.n_q; ++i) ++cnt_items[i];
+        cnt_it0 += (g.n_q >= 1);
+        cnt_it1 += (g.n_q >= 2);
         }
         // K/V tiles only the cluster partner needs (it sees more chunk frames, or this CTA has no query rows)
         for (int e = 2 * g.n_kv; e < 2 * g.n_pipe; ++e) {
@@ -360,7 +363,6 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
     const uint32_t taddr_o = tmem_base + lane_sel + 256 + wg * D;
     const float c = p.scale_log2;
     const float thr = kRescaleThresholdLog2 / c;
-    const uint32_t taddr_o_other = tmem_base + lane_sel + 256 + (wg ^ 1) * D;
     uint32_t cnt_s = 0, cnt_pv = 0;
     uint32_t cnt_pv_other = 0;                            // PV groups committed so far on the OTHER tile slot
     for (int idx = it_begin; idx < it_end; ++idx) {
@@ -520,6 +522,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
         mbar_wait(&o_done[wg ^ 1], (cnt_pv_other - 1) & 1);
         tc_fence_after();
         const int col0 = wg * (D / 2);
+        const uint32_t taddr_o_other = tmem_base + lane_sel + 256 + (wg ^ 1) * D;
 #pragma unroll
         for (int cc = 0; cc < D / 2; cc += 32) {
           uint32_t o[32], q[32];
