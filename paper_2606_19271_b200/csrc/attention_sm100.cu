@@ -55,8 +55,28 @@ struct ItemGeom {
   bool split;   // lone query tile: its KV tiles alternate between the two TMEM tile slots (even / odd), merged at the end
 };
 
-__device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int idx) {
-  const WorkItem w = p.items[idx];
+// Cluster items are handed out dynamically, in the host's (session, head) stream order: the TMA thread of CTA rank 0
+// takes the next one from a global cursor when it gets there (it runs ahead of every other role) and publishes it as
+// the k-th item of its cluster; every other role of both CTAs reads entry k of the cluster's ring.  An entry carries
+// its sequence number, so a stale value of the ring slot's previous use is never mistaken for it.  -1: no more items.
+__device__ __forceinline__ int next_cluster_item(const AttnParams& p, uint32_t k, bool fetcher) {
+  unsigned long long* slot = p.feed + (size_t)(blockIdx.x >> 1) * kFeedRing + (k % kFeedRing);
+  if (fetcher) {
+    int idx = atomicAdd(p.feed_counter, 1);
+    if (idx >= p.n_citems) idx = -1;
+    const unsigned long long v = ((unsigned long long)(k + 1) << 32) | (uint32_t)(idx + 1);
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(slot), "l"(v) : "memory");
+    return idx;
+  }
+  unsigned long long v;
+  do {
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(slot) : "memory");
+  } while ((uint32_t)(v >> 32) != k + 1);
+  return (int)(uint32_t)v - 1;
+}
+
+__device__ __forceinline__ ItemGeom decode_item(const AttnParams& p, int citem, uint32_t cta_rank) {
+  const WorkItem w = p.items[2 * citem + cta_rank];
   const SessDesc s = p.sess[w.sess];
   ItemGeom g;
   g.sess = w.sess;
@@ -141,8 +161,6 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
   const uint32_t cta_rank = cluster_ctarank();
   const uint32_t tmem_base = *tmem_ptr;
 
-  const int it_begin = p.cta_begin[blockIdx.x];
-  const int it_end = p.cta_begin[blockIdx.x + 1];
 
   if (warp < 4) {
     setmaxnreg_dec<kRegsProducer>();
@@ -153,8 +171,10 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
       uint32_t q_cnt = 0;
       const int sb = min(p.B, 64);            // tokens per TMA box of K/V (the maps are encoded with this box)
       const int n_sub = 128 / sb;             // boxes per 128-key tile
-      for (int idx = it_begin; idx < it_end; ++idx) {
-        const ItemGeom g = decode_item(p, idx);
+      for (uint32_t k_item = 0;; ++k_item) {
+        const int idx = next_cluster_item(p, k_item, cta_rank == 0);
+        if (idx < 0) break;
+        const ItemGeom g = decode_item(p, idx, cta_rank);
         const CUtensorMap* mq = p.sess_maps + g.sess * 3;
         const CUtensorMap* mkn = mq + 1;
         const CUtensorMap* mvn = mq + 2;
@@ -237,8 +257,10 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
       uint32_t kv_it = 0, q_cnt = 0;
       // per tile slot: P hand-offs and items so far (scalars with selects: a runtime-indexed array would live in local memory)
       uint32_t cnt_p0 = 0, cnt_p1 = 0, cnt_it0 = 0, cnt_it1 = 0;
-      for (int idx = it_begin; idx < it_end; ++idx) {
-        const ItemGeom g = decode_item(p, idx);
+      for (uint32_t k_item = 0;; ++k_item) {
+        const int idx = next_cluster_item(p, k_item, false);
+        if (idx < 0) break;
+        const ItemGeom g = decode_item(p, idx, cta_rank);
         // hand a K/V slot back once every MMA issued so far has read it - always to BOTH CTAs of the cluster, also
         // when the two work on unrelated items: a slot is refilled (possibly by the partner's multicast) only after
         // both CTAs are done with their tile at that ring position
@@ -365,8 +387,10 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
     const float thr = kRescaleThresholdLog2 / c;
     uint32_t cnt_s = 0, cnt_pv = 0;
     uint32_t cnt_pv_other = 0;                            // PV groups committed so far on the OTHER tile slot
-    for (int idx = it_begin; idx < it_end; ++idx) {
-      const ItemGeom g = decode_item(p, idx);
+    for (uint32_t k_item = 0;; ++k_item) {
+      const int idx = next_cluster_item(p, k_item, false);
+      if (idx < 0) break;
+      const ItemGeom g = decode_item(p, idx, cta_rank);
       if (!g.split && wg >= g.n_q) {
         if (g.n_q == 1) cnt_pv_other += g.n_kv;           // warpgroup 1 sits out a lone tile that runs on slot 0 alone
         continue;

@@ -35,6 +35,8 @@ struct WorkItem {      // one (session, head, one or two 128-row query tiles) fo
 };
 static_assert(sizeof(WorkItem) == 16, "WorkItem layout");
 
+constexpr int kFeedRing = 16;   // entries of a cluster's item-feed ring
+
 struct AttnParams {
   CUtensorMap map_k;             // this layer's cached K: 4D {D, B, H, n_pages}
   CUtensorMap map_v;             // this layer's cached V
@@ -42,7 +44,9 @@ struct AttnParams {
   const SessDesc* sess;
   const int32_t* page_tables;
   const WorkItem* items;
-  const int32_t* cta_begin;      // [grid + 1] item ranges per CTA (LPT-balanced on the host)
+  unsigned long long* feed;      // [grid/2][kFeedRing] per-cluster ring of (sequence number, cluster item) pairs and
+  int32_t* feed_counter;         // the global cursor into the cluster-item list: see next_cluster_item()
+  int32_t n_citems;              // cluster items; items[2*i + r] is the work of CTA rank r for cluster item i
   uint16_t* out;                 // bf16 [sum C][H][D]
   float* lse;                    // fp32 [sum C][H] or null
   int32_t H, T, B, log2_B;

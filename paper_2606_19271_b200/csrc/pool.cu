@@ -637,14 +637,12 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
       Plan fine = make_plan(1);
       if (fine.makespan * 108 < plan.makespan * 100) plan = std::move(fine);   // single tiles cost ~8 % more per FLOP
     }
-    const int grid = 2 * (int)plan.per_cluster.size();
-    cta_begin.assign(grid + 1, 0);
+    // The kernel hands cluster items out dynamically in THIS order (a global cursor): clusters that run a little
+    // faster simply take more; the list-scheduling above only serves to compare the two plans.
     items.clear();
-    for (int ci = 0; ci < grid; ++ci) {
-      cta_begin[ci] = (int32_t)items.size();
-      for (int i : plan.per_cluster[ci >> 1]) {
-        const CItem& it = plan.citems[i];
-        const Cand& x = (ci & 1) ? it.b : it.a;
+    for (const CItem& it : plan.citems) {
+      for (int r = 0; r < 2; ++r) {
+        const Cand& x = r ? it.b : it.a;
         WorkItem wi;
         wi.sess = x.sess;
         wi.head = x.head;
@@ -653,10 +651,12 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
         items.push_back(wi);
       }
     }
-    cta_begin[grid] = (int32_t)items.size();
+    cta_begin.assign(1, 2 * (int)plan.per_cluster.size());   // [0] = grid
     pool->sched_key = key;
   }
-  const int grid = (int)pool->sched_cta.size() - 1;
+  const int grid = pool->sched_cta[0];
+  const int n_citems = (int)pool->sched_items.size() / 2;
+  const size_t feed_bytes = 128 + (size_t)(grid / 2) * kFeedRing * 8;   // cursor + per-cluster rings, zeroed per call
   ScheduleLayout L;
   L.n_items = (int)pool->sched_items.size();
   L.grid = grid;
@@ -664,7 +664,7 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   L.off_sess = align_up(L.off_maps + (size_t)n * 3 * sizeof(CUtensorMap), 128);
   L.off_pt = align_up(L.off_sess + (size_t)n * sizeof(SessDesc), 128);
   L.off_cta = align_up(L.off_pt + pool->sched_pt.size() * 4, 128);
-  L.off_items = align_up(L.off_cta + (size_t)(grid + 1) * 4, 128);
+  L.off_items = align_up(L.off_cta + feed_bytes, 128);
   L.bytes = L.off_items + pool->sched_items.size() * sizeof(WorkItem);
   Staging* st = nullptr;
   rc = acquire_staging(pool, L.bytes, &st);
@@ -672,7 +672,7 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   CUtensorMap* maps = reinterpret_cast<CUtensorMap*>(st->h + L.off_maps);
   memcpy(st->h + L.off_sess, pool->sched_sess.data(), (size_t)n * sizeof(SessDesc));
   memcpy(st->h + L.off_pt, pool->sched_pt.data(), pool->sched_pt.size() * 4);
-  memcpy(st->h + L.off_cta, pool->sched_cta.data(), (size_t)(grid + 1) * 4);
+  memset(st->h + L.off_cta, 0, feed_bytes);
   memcpy(st->h + L.off_items, pool->sched_items.data(), pool->sched_items.size() * sizeof(WorkItem));
   for (int b = 0; b < n; ++b) {
     // per-session 3D maps {D, H, C}: rows past the session's chunk read as zeros, never as a neighbour's tokens
@@ -697,7 +697,9 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   p.sess_maps = reinterpret_cast<const CUtensorMap*>(st->d + L.off_maps);
   p.sess = reinterpret_cast<const SessDesc*>(st->d + L.off_sess);
   p.page_tables = reinterpret_cast<const int32_t*>(st->d + L.off_pt);
-  p.cta_begin = reinterpret_cast<const int32_t*>(st->d + L.off_cta);
+  p.feed_counter = reinterpret_cast<int32_t*>(st->d + L.off_cta);
+  p.feed = reinterpret_cast<unsigned long long*>(st->d + L.off_cta + 128);
+  p.n_citems = n_citems;
   p.items = reinterpret_cast<const WorkItem*>(st->d + L.off_items);
   p.out = (uint16_t*)out;
   p.lse = lse;
