@@ -156,9 +156,9 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*
  * One coalesced chunk step with DEVICE buffers: ts_chunk_attention followed by ts_kv_append(flags) as one call
  * (PAPER.md:66 (iii): "invokes the model once for the batch ... writes ... updated states back").  Results are those
  * of the two calls in sequence.  The append writes cache slots this step's attention does not read (R5) and is
- * HBM-bound while the attention is tensor-bound, so it runs on a stream of the pool UNDER the attention kernel;
- * `cuda_stream` waits for both, and everything the pool remembers about completion is recorded on `cuda_stream`.
- * Arguments as in the two calls.  All-or-nothing: page demand is checked before anything is enqueued.
+ * HBM-bound while the attention is not, so it is carried out INSIDE the attention launch, by the two warps of every
+ * CTA that have no other role: one kernel, and the step takes what the attention takes.
+ * Arguments as in the two calls.  All-or-nothing: arguments and page demand are checked before anything changes.
  */
 int ts_chunk_step(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*host*/,
                   const int32_t* chunk_frames /*host*/, const void* q, const void* k, const void* v, void* out,

@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libturbochunk.so")
 SOURCES = ["pool.cu", "kv_copy.cu", "attention_sm100.cu"]
-HEADERS = ["internal.h", "ptx.cuh", os.path.join("..", "..", "include", "turbochunk.h")]
+HEADERS = ["internal.h", "ptx.cuh", "kv_copy.cuh", os.path.join("..", "..", "include", "turbochunk.h")]
 
 
 def _stale():

@@ -9,6 +9,7 @@
 // Warp roles (384 threads):
 //   warp 0      TMA producer   Q tiles once per item, K/V tiles into a ring of kSlots smem slots
 //   warp 1      MMA issuer     tcgen05.mma, one elected thread; S = Q K^T (SS), O += P V (TS, P in TMEM)
+//   warps 2-3   idle, or (fused chunk step) the KV append of the batch: 128-bit streaming copies into the pages
 //   warps 4-7   softmax for query tile 0 (one thread per row): online softmax in fp32, lazy rescale of O,
 //   warps 8-11  softmax for query tile 1                        P written back to TMEM as bf16, epilogue
 // TMEM (512 columns): S0 [0,128) / P0 aliases [0,64); S1 [128,256) / P1; O0 [256,256+D); O1 [256+D,256+2D).
@@ -21,6 +22,7 @@
 // the same number of tiles through their rings so that a tile sits at the same smem offset in both.  Every slot
 // release goes to the kv_empty barriers of both CTAs (count 2), also when the two CTAs work on unrelated items.
 #include "internal.h"
+#include "kv_copy.cuh"
 #include "ptx.cuh"
 
 namespace tc {
@@ -374,6 +376,11 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
         }
       }
     }
+  } else if (p.copy.n_sess > 0) {
+    // ===================================================================== warps 2-3: KV append of a fused chunk step
+    // The append writes cache slots this launch's attention never reads (R5); it is HBM-bound and the attention is not,
+    // so it costs the step nothing when it runs here, under the attention.
+    append_by_workers(p.copy, (int64_t)blockIdx.x * 64 + (threadIdx.x - 64), (int64_t)gridDim.x * 64);
   }
   } else {
     setmaxnreg_inc<kRegsSoftmax>();

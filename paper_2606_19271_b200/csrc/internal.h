@@ -35,25 +35,6 @@ struct WorkItem {      // one (session, head, one or two 128-row query tiles) fo
 };
 static_assert(sizeof(WorkItem) == 16, "WorkItem layout");
 
-constexpr int kFeedRing = 16;   // entries of a cluster's item-feed ring
-
-struct AttnParams {
-  CUtensorMap map_k;             // this layer's cached K: 4D {D, B, H, n_pages}
-  CUtensorMap map_v;             // this layer's cached V
-  const CUtensorMap* sess_maps;  // device [n][3]: per-session Q, Kn, Vn maps (3D {D, H, C_s}); OOB rows zero-fill
-  const SessDesc* sess;
-  const int32_t* page_tables;
-  const WorkItem* items;
-  unsigned long long* feed;      // [grid/2][kFeedRing] per-cluster ring of (sequence number, cluster item) pairs and
-  int32_t* feed_counter;         // the global cursor into the cluster-item list: see next_cluster_item()
-  int32_t n_citems;              // cluster items; items[2*i + r] is the work of CTA rank r for cluster item i
-  uint16_t* out;                 // bf16 [sum C][H][D]
-  float* lse;                    // fp32 [sum C][H] or null
-  int32_t H, T, B, log2_B;
-  float scale_log2;              // scale * log2(e)
-  float scale;
-};
-
 struct CopySess {      // append / gather descriptor
   int32_t tok_off;     // first token in the packed source (append) / 0 (gather)
   int32_t n_tok;       // tokens to copy
@@ -79,6 +60,27 @@ struct CopyParams {
   const uint8_t* src_v;
   uint8_t* dst_k;           // gather: logical [L][H][D] output
   uint8_t* dst_v;
+};
+
+constexpr int kFeedRing = 16;   // entries of a cluster's item-feed ring
+
+struct AttnParams {
+  CUtensorMap map_k;             // this layer's cached K: 4D {D, B, H, n_pages}
+  CUtensorMap map_v;             // this layer's cached V
+  const CUtensorMap* sess_maps;  // device [n][3]: per-session Q, Kn, Vn maps (3D {D, H, C_s}); OOB rows zero-fill
+  const SessDesc* sess;
+  const int32_t* page_tables;
+  const WorkItem* items;
+  unsigned long long* feed;      // [grid/2][kFeedRing] per-cluster ring of (sequence number, cluster item) pairs and
+  int32_t* feed_counter;         // the global cursor into the cluster-item list: see next_cluster_item()
+  int32_t n_citems;              // cluster items; items[2*i + r] is the work of CTA rank r for cluster item i
+  uint16_t* out;                 // bf16 [sum C][H][D]
+  float* lse;                    // fp32 [sum C][H] or null
+  int32_t H, T, B, log2_B;
+  float scale_log2;              // scale * log2(e)
+  float scale;
+  CopyParams copy;               // fused chunk step: the KV append, done by the two idle warps of every CTA
+                                 // (copy.n_sess == 0: none)
 };
 
 // kernel launchers (return cudaGetLastError())

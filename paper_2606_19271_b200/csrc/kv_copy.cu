@@ -3,31 +3,12 @@
 // (contiguous [tokens][H][D]) and in 2*D-byte runs on the paged side ([page][layer][K|V][H][B][D]).
 // HBM-bound: algorithmic bytes = read + write of K and V = 4 * tokens * H * D * 2.
 #include "internal.h"
+#include "kv_copy.cuh"
 
 namespace tc {
 
 constexpr int kCopyThreads = 256;
 constexpr int kCopyUnroll = 4;
-
-__device__ __forceinline__ uint4 ld_stream(const void* p) {
-  uint4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-  return r;
-}
-
-// Byte offset inside the slab (relative to the layer's K or V block of the page) of 16-byte element `e`
-// of a session, where e indexes [row][H][D/8] and row is relative to x0.
-__device__ __forceinline__ int64_t paged_offset(const CopyParams& p, const CopySess& s, const int32_t* pt, int64_t e,
-                                                int vec_per_head, int vec_per_row) {
-  const int row = (int)(e / vec_per_row);
-  const int rem = (int)(e - (int64_t)row * vec_per_row);
-  const int h = rem / vec_per_head;
-  const int v = rem - h * vec_per_head;
-  const int x = s.x0 + row;
-  const int page = pt[x >> p.log2_B];
-  const int slot = x & (p.B - 1);
-  return (int64_t)page * p.page_stride + ((int64_t)h * p.B + slot) * (p.D * 2) + v * 16;
-}
 
 __global__ void __launch_bounds__(kCopyThreads) kv_append_kernel(const CopyParams p) {
   const CopySess s = p.sess[blockIdx.y];

@@ -135,8 +135,6 @@ struct ts_pool {
   cudaStream_t h2d_s = nullptr, d2h_s = nullptr;   // ... its copy streams (input of step t+1 overlaps step t)
   cudaEvent_t ev_in = nullptr, ev_attn = nullptr, ev_out = nullptr, ev_free[2] = {nullptr, nullptr};
   uint64_t host_steps = 0;
-  cudaStream_t aux_s = nullptr;            // ts_chunk_step: the append runs here, under the attention kernel
-  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   size_t stage_cap = 0;
   int64_t launches = 0;
   std::vector<int32_t> scratch_mark;       // duplicate detection
@@ -292,9 +290,6 @@ int ts_pool_destroy(ts_pool* pool) {
   if (pool->stage_dev) cudaFree(pool->stage_dev);
   if (pool->h2d_s) cudaStreamDestroy(pool->h2d_s);
   if (pool->d2h_s) cudaStreamDestroy(pool->d2h_s);
-  if (pool->aux_s) cudaStreamDestroy(pool->aux_s);
-  if (pool->ev_fork) cudaEventDestroy(pool->ev_fork);
-  if (pool->ev_join) cudaEventDestroy(pool->ev_join);
   for (cudaEvent_t e : {pool->ev_in, pool->ev_attn, pool->ev_out, pool->ev_free[0], pool->ev_free[1]})
     if (e) cudaEventDestroy(e);
   pool->tl_compute.destroy();
@@ -478,8 +473,17 @@ void* ts_pool_side_stream(ts_pool* pool) { return pool ? (void*)pool->side : nul
 int64_t ts_pool_launch_count(ts_pool* pool) { return pool ? pool->launches : 0; }
 
 // --------------------------------------------------------------------------------------------- attention
-int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
-                       const void* q, const void* k, const void* v, void* out, float* lse, float scale, void* cuda_stream) {
+// The KV append of a fused chunk step, prepared on the host (pages already allocated) and carried out by the idle
+// warps of the attention kernel.
+struct FusedAppend {
+  std::vector<CopySess> cs;            // pt_off is filled in from the attention schedule (same packed page tables)
+  uint64_t wait_side = 0, wait_compute = 0;
+  int total_rows = 0;
+};
+
+static int attention_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
+                          const void* q, const void* k, const void* v, void* out, float* lse, float scale,
+                          void* cuda_stream, const FusedAppend* fused, uint64_t* seq_out) {
   if (pool == nullptr) return TS_ERR_INVALID;
   int rc = check_batch(pool, layer, n, sids, chunk_frames);
   if (rc != TS_OK) return rc;
@@ -665,7 +669,8 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   L.off_pt = align_up(L.off_sess + (size_t)n * sizeof(SessDesc), 128);
   L.off_cta = align_up(L.off_pt + pool->sched_pt.size() * 4, 128);
   L.off_items = align_up(L.off_cta + feed_bytes, 128);
-  L.bytes = L.off_items + pool->sched_items.size() * sizeof(WorkItem);
+  const size_t off_copy = align_up(L.off_items + pool->sched_items.size() * sizeof(WorkItem), 128);
+  L.bytes = off_copy + (fused ? (size_t)n * sizeof(CopySess) : 0);
   Staging* st = nullptr;
   rc = acquire_staging(pool, L.bytes, &st);
   if (rc != TS_OK) return rc;
@@ -674,6 +679,13 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   memcpy(st->h + L.off_pt, pool->sched_pt.data(), pool->sched_pt.size() * 4);
   memset(st->h + L.off_cta, 0, feed_bytes);
   memcpy(st->h + L.off_items, pool->sched_items.data(), pool->sched_items.size() * sizeof(WorkItem));
+  if (fused) {
+    CopySess* cs = reinterpret_cast<CopySess*>(st->h + off_copy);
+    for (int b = 0; b < n; ++b) {
+      cs[b] = fused->cs[b];
+      cs[b].pt_off = pool->sched_sess[b].pt_off;
+    }
+  }
   for (int b = 0; b < n; ++b) {
     // per-session 3D maps {D, H, C}: rows past the session's chunk read as zeros, never as a neighbour's tokens
     const SessDesc& d = pool->sched_sess[b];
@@ -689,9 +701,30 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
 
   // ---- ordering: wait (stream-side) for pending resumes of the batch's sessions
   for (int b = 0; b < n; ++b) TS_CUDA(pool->tl_side.wait(stream, pool->sess[sids[b]].side_seq));
+  if (fused) {   // ... and for copies out of / readers of the pages the append is about to write
+    TS_CUDA(pool->tl_side.wait(stream, fused->wait_side));
+    TS_CUDA(pool->tl_compute.wait(stream, fused->wait_compute));
+  }
 
   TS_CUDA(cudaMemcpyAsync(st->d, st->h, L.bytes, cudaMemcpyHostToDevice, stream));
   AttnParams p;
+  memset(&p.copy, 0, sizeof(p.copy));
+  if (fused) {
+    p.copy.sess = reinterpret_cast<const CopySess*>(st->d + off_copy);
+    p.copy.page_tables = reinterpret_cast<const int32_t*>(st->d + L.off_pt);
+    p.copy.n_sess = n;
+    p.copy.total_rows = fused->total_rows;
+    p.copy.H = H;
+    p.copy.D = D;
+    p.copy.B = c.page_tokens;
+    p.copy.log2_B = pool->log2_B;
+    p.copy.page_stride = pool->page_bytes;
+    p.copy.layer_k_off = (int64_t)layer * pool->layer_bytes;
+    p.copy.layer_v_off = p.copy.layer_k_off + pool->kv_bytes;
+    p.copy.slab = pool->slab;
+    p.copy.src_k = (const uint8_t*)k;
+    p.copy.src_v = (const uint8_t*)v;
+  }
   p.map_k = pool->map_k[layer];
   p.map_v = pool->map_v[layer];
   p.sess_maps = reinterpret_cast<const CUtensorMap*>(st->d + L.off_maps);
@@ -715,14 +748,45 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   st->in_flight = true;
   const uint64_t seq = pool->tl_compute.record(stream);
   for (int b = 0; b < n; ++b) pool->sess[sids[b]].compute_seq = seq;
+  if (seq_out) *seq_out = seq;
   return TS_OK;
 }
 
+int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
+                       const void* q, const void* k, const void* v, void* out, float* lse, float scale, void* cuda_stream) {
+  return attention_impl(pool, layer, n, sids, chunk_frames, q, k, v, out, lse, scale, cuda_stream, nullptr, nullptr);
+}
+
 // --------------------------------------------------------------------------------------------- append
-// Append on `exec`; when `join` is another stream, `join` waits for the append and the completion that sessions and
-// freed pages remember is recorded on `join` (after everything enqueued there so far, e.g. the attention of the step).
-static int append_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames, const void* k,
-                       const void* v, uint32_t flags, cudaStream_t stream, cudaStream_t join) {
+// Host bookkeeping after an append has been enqueued (its completion is `seq` on the compute timeline): with
+// TS_COMMIT the sessions grow by their chunk and the window rolls (a4).
+static void append_commit(ts_pool* pool, int32_t n, const int32_t* sids, const int32_t* chunk_frames, uint32_t flags,
+                          uint64_t seq) {
+  const int T = pool->cfg.frame_tokens, B = pool->cfg.page_tokens, W = pool->cfg.window_frames;
+  for (int b = 0; b < n; ++b) {
+    Session& s = pool->sess[sids[b]];
+    s.compute_seq = seq;
+    if (flags & TS_COMMIT) {
+      s.ver = ++pool->ver_seq;
+      s.P += chunk_frames[b];
+      const int e = W > 0 ? std::max(0, s.P - W) : 0;   // a4: evict oldest whole frames (R6 ii, R10)
+      s.P -= e;
+      s.o += e * T;
+      while (s.o >= B) {
+        const int32_t pg = s.pt.front();
+        s.pt.erase(s.pt.begin());
+        pool->page_compute_seq[pg] = seq;
+        pool->page_side_seq[pg] = s.side_seq;
+        pool->free_q.push_back(pg);
+        s.o -= B;
+      }
+    }
+  }
+}
+
+int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames, const void* k,
+                 const void* v, uint32_t flags, void* cuda_stream) {
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
   if (pool == nullptr) return TS_ERR_INVALID;
   int rc = check_batch(pool, layer, n, sids, chunk_frames);
   if (rc != TS_OK) return rc;
@@ -731,7 +795,7 @@ static int append_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   if ((flags & ~(uint32_t)TS_COMMIT) != 0) return TS_ERR_INVALID;
   const ts_pool_config& c = pool->cfg;
   TS_CUDA(cudaSetDevice(c.device));
-  const int T = c.frame_tokens, B = c.page_tokens, W = c.window_frames;
+  const int T = c.frame_tokens, B = c.page_tokens;
 
   // demand check first: all-or-nothing (O2)
   std::vector<int> need(n);
@@ -807,37 +871,10 @@ static int append_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   ++pool->launches;
   TS_CUDA(cudaEventRecord(st->ev, stream));
   st->in_flight = true;
-  if (join != stream) {
-    TS_CUDA(cudaEventRecord(pool->ev_join, stream));
-    TS_CUDA(cudaStreamWaitEvent(join, pool->ev_join, 0));
-  }
-  const uint64_t seq = pool->tl_compute.record(join);
+  const uint64_t seq = pool->tl_compute.record(stream);
 
-  for (int b = 0; b < n; ++b) {
-    Session& s = pool->sess[sids[b]];
-    s.compute_seq = seq;
-    if (flags & TS_COMMIT) {
-      s.ver = ++pool->ver_seq;
-      s.P += chunk_frames[b];
-      const int e = W > 0 ? std::max(0, s.P - W) : 0;   // a4: evict oldest whole frames (R6 ii, R10)
-      s.P -= e;
-      s.o += e * T;
-      while (s.o >= B) {
-        const int32_t pg = s.pt.front();
-        s.pt.erase(s.pt.begin());
-        pool->page_compute_seq[pg] = seq;
-        pool->page_side_seq[pg] = s.side_seq;
-        pool->free_q.push_back(pg);
-        s.o -= B;
-      }
-    }
-  }
+  append_commit(pool, n, sids, chunk_frames, flags, seq);
   return TS_OK;
-}
-
-int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames, const void* k,
-                 const void* v, uint32_t flags, void* cuda_stream) {
-  return append_impl(pool, layer, n, sids, chunk_frames, k, v, flags, (cudaStream_t)cuda_stream, (cudaStream_t)cuda_stream);
 }
 
 // --------------------------------------------------------------------------------------------- fused device step
@@ -847,32 +884,56 @@ int ts_chunk_step(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, 
   int rc = check_batch(pool, layer, n, sids, chunk_frames);
   if (rc != TS_OK) return rc;
   if (n == 0) return TS_OK;
-  if (k == nullptr || v == nullptr || (((uintptr_t)k | (uintptr_t)v) & 15) != 0) return TS_ERR_INVALID;
+  if (q == nullptr || k == nullptr || v == nullptr || out == nullptr) return TS_ERR_INVALID;
+  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) != 0) return TS_ERR_INVALID;
+  if (!(scale > 0.0f) || !std::isfinite(scale)) return TS_ERR_INVALID;
   if ((flags & ~(uint32_t)TS_COMMIT) != 0) return TS_ERR_INVALID;
-  {   // page demand of the append, before anything is enqueued (all-or-nothing)
-    const int T = pool->cfg.frame_tokens, B = pool->cfg.page_tokens;
-    int64_t need_total = 0;
-    for (int b = 0; b < n; ++b) {
-      const Session& s = pool->sess[sids[b]];
-      const int64_t end = (int64_t)s.o + (int64_t)s.P * T + (int64_t)chunk_frames[b] * T;
-      need_total += std::max<int64_t>(0, (end + B - 1) / B - (int64_t)s.pt.size());
+  const int T = pool->cfg.frame_tokens, B = pool->cfg.page_tokens;
+  // page demand of the append, before anything changes or is enqueued (all-or-nothing, O2)
+  std::vector<int> need(n);
+  int64_t need_total = 0;
+  for (int b = 0; b < n; ++b) {
+    const Session& s = pool->sess[sids[b]];
+    const int64_t end = (int64_t)s.o + (int64_t)s.P * T + (int64_t)chunk_frames[b] * T;
+    need[b] = (int)std::max<int64_t>(0, (end + B - 1) / B - (int64_t)s.pt.size());
+    need_total += need[b];
+  }
+  if (need_total > (int64_t)pool->free_q.size()) return TS_ERR_NO_PAGES;
+  // grow the page tables first: the attention schedule is then built from the grown tables (the attention itself only
+  // reads [x_begin, x_end), R5) and its packed page-table array also serves the append, which the idle warps of the
+  // attention kernel carry out - it is HBM-bound, the attention is not, so it costs the step nothing there
+  FusedAppend fa;
+  fa.cs.resize(n);
+  int tok_off = 0, row_off = 0;
+  for (int b = 0; b < n; ++b) {
+    Session& s = pool->sess[sids[b]];
+    if (need[b] > 0) s.ver = ++pool->ver_seq;
+    for (int i = 0; i < need[b]; ++i) {
+      const int32_t pg = pool->free_q.front();
+      pool->free_q.pop_front();
+      fa.wait_side = std::max(fa.wait_side, pool->page_side_seq[pg]);        // a D2H copy out of the page may be pending
+      fa.wait_compute = std::max(fa.wait_compute, pool->page_compute_seq[pg]);
+      s.pt.push_back(pg);
     }
-    if (need_total > (int64_t)pool->free_q.size()) return TS_ERR_NO_PAGES;
+    const int C = chunk_frames[b] * T;
+    const int x0 = s.o + s.P * T;
+    CopySess& d = fa.cs[b];
+    d.tok_off = tok_off;
+    d.n_tok = C;
+    d.n_zero = (B - ((x0 + C) & (B - 1))) & (B - 1);
+    d.x0 = x0;
+    d.pt_off = 0;
+    d.row_off = row_off;
+    d.pad0 = d.pad1 = 0;
+    tok_off += C;
+    row_off += d.n_tok + d.n_zero;
   }
-  cudaStream_t stream = (cudaStream_t)cuda_stream;
-  TS_CUDA(cudaSetDevice(pool->cfg.device));
-  if (pool->aux_s == nullptr) {
-    TS_CUDA(cudaStreamCreateWithFlags(&pool->aux_s, cudaStreamNonBlocking));
-    TS_CUDA(cudaEventCreateWithFlags(&pool->ev_fork, cudaEventDisableTiming));
-    TS_CUDA(cudaEventCreateWithFlags(&pool->ev_join, cudaEventDisableTiming));
-  }
-  // The append writes slots [L, L+C) that this step's attention does not read (R5), and it is HBM-bound while the
-  // attention is tensor-bound: it runs on a second stream under the attention kernel and joins `cuda_stream` after it.
-  TS_CUDA(cudaEventRecord(pool->ev_fork, stream));
-  TS_CUDA(cudaStreamWaitEvent(pool->aux_s, pool->ev_fork, 0));
-  rc = ts_chunk_attention(pool, layer, n, sids, chunk_frames, q, k, v, out, lse, scale, cuda_stream);
+  fa.total_rows = row_off;
+  uint64_t seq = 0;
+  rc = attention_impl(pool, layer, n, sids, chunk_frames, q, k, v, out, lse, scale, cuda_stream, &fa, &seq);
   if (rc != TS_OK) return rc;
-  return append_impl(pool, layer, n, sids, chunk_frames, k, v, flags, pool->aux_s, stream);
+  append_commit(pool, n, sids, chunk_frames, flags, seq);
+  return TS_OK;
 }
 
 // --------------------------------------------------------------------------------------------- gather
