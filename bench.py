@@ -6,8 +6,8 @@
 One JSON line on stdout (rank 0).  A "step" is one pass of the hot path over one coalesced batch:
     resume(idle session X) on the side stream                      (a6)
     open + close of a transient session                            (a7)
-    ts_chunk_step(batch of 8, flags=0)    scheduler + attention (a1, a2) and paged scatter (a3), the scatter
-                                          running under the attention kernel on a stream of the pool
+    ts_chunk_step(batch of 8, flags=0)    scheduler + attention (a1, a2) and paged scatter (a3) in ONE launch: the
+                                          scatter is done by the two role-less warps of every attention CTA
     suspend(X) on the side stream                                  (a5)
 flags=0 keeps every timed step on the identical drawn state of configs[2]; the window roll (a4) is host
 integer arithmetic inside ts_kv_append(TS_COMMIT), exercised by the tests, not by the timed loop.
