@@ -37,7 +37,7 @@ NOMINAL_BF16_TFLOPS = 2250.0
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one attention launch on this workload, from the ncu --set full
 # capture summarised in profiles/ (None until a capture exists).
-ATTENTION_DRAM_TRAFFIC_BYTES = 1120753544  # 1013.41 MB read + 107.34 MB write, profiles/r1_attention_final.txt
+ATTENTION_DRAM_TRAFFIC_BYTES = 1074712320  # 970.98 MB read + 103.74 MB write (attention-only launch), profiles/r1_attention_final.txt
 
 
 def load_peaks():
