@@ -36,6 +36,31 @@ constexpr int kRegsProducer = 72;
 constexpr int kRegsSoftmax = 216;
 static_assert(128 * kRegsProducer + 256 * kRegsSoftmax <= 384 * 168, "register pool");
 
+// One MUFU.EX2 per score costs exactly as many SM cycles as the score's two MMAs at D = 128 (16/clk/SM against 8192
+// FLOP/clk/SM), and the exp phase of a tile sits on the S -> softmax -> PV -> S chain.  kPolyPairs of every 16 score
+// pairs are therefore evaluated on the FMA pipe instead.  One warp owns a tile's rows, so the instructions this adds
+// (11 per pair against 2 MUFU) soon make the phase issue-bound: measured on configs[2], 4 of 16 is the optimum (+1.3 %),
+// 6 of 16 already loses.
+constexpr int kPolyPairs = 4;
+
+// 2^x for a pair on the FMA pipe (Cody-Waite): x = n + f with n = round(x), f in [-0.5, 0.5]; 2^f by a degree-3 minimax
+// polynomial (max relative error 7.5e-5, far below the 2^-9 of the bf16 rounding of P); 2^n as the fp32 whose bits are
+// (n + 127) << 23 - n + 127 sits in the low mantissa bits of x + (1.5 * 2^23 + 127).  x is clamped at -125 (masked
+// scores are -inf), which yields 2^-125 instead of 0: negligible against a row sum >= 1.
+__device__ __forceinline__ void exp2_poly_pair(float x0, float x1, float& p0, float& p1) {
+  x0 = fmaxf(x0, -125.f);
+  x1 = fmaxf(x1, -125.f);
+  float f0, f1, n0, n1, r0, r1, q0, q1;
+  addc2(f0, f1, x0, x1, 12583039.f);
+  addc2(n0, n1, f0, f1, -12583039.f);
+  sub2(r0, r1, x0, x1, n0, n1);
+  fma2_bcast(q0, q1, r0, r1, 0.05517083778977394f, 0.24260935187339783f);
+  fma2_pc(q0, q1, q0, q1, r0, r1, 0.6932609677314758f);
+  fma2_pc(q0, q1, q0, q1, r0, r1, 0.9999281764030457f);
+  p0 = q0 * __uint_as_float(shl_alu(__float_as_uint(f0), 23));
+  p1 = q1 * __uint_as_float(shl_alu(__float_as_uint(f1), 23));
+}
+
 template <int D>
 struct Cfg {
   static constexpr int kTileBytes = 128 * D * 2;        // one [128 x D] bf16 tile
@@ -489,7 +514,14 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
             float x0, x1, x2, x3;
             fma2_bcast(x0, x1, __uint_as_float(s[cc + k]), __uint_as_float(s[cc + k + 1]), c, neg_mc);
             fma2_bcast(x2, x3, __uint_as_float(s[cc + k + 2]), __uint_as_float(s[cc + k + 3]), c, neg_mc);
-            const float p0 = ex2_approx(x0), p1 = ex2_approx(x1), p2 = ex2_approx(x2), p3 = ex2_approx(x3);
+            float p0, p1, p2, p3;
+            {
+              const int pj = k >> 1;   // index of (x0, x1) among the 16 pairs of this 32-column chunk
+              if (((pj + 1) * kPolyPairs) / 16 != (pj * kPolyPairs) / 16) exp2_poly_pair(x0, x1, p0, p1);
+              else { p0 = ex2_approx(x0); p1 = ex2_approx(x1); }
+              if (((pj + 2) * kPolyPairs) / 16 != ((pj + 1) * kPolyPairs) / 16) exp2_poly_pair(x2, x3, p2, p3);
+              else { p2 = ex2_approx(x2); p3 = ex2_approx(x3); }
+            }
             add2(l0, l1, p0, p1);
             add2(l2, l3, p2, p3);
             pk[k >> 1] = pack_bf16x2(p0, p1);

@@ -269,6 +269,49 @@ __device__ __forceinline__ void mul2_bcast(float& d0, float& d1, float a0, float
       : "=f"(d0), "=f"(d1)
       : "f"(a0), "f"(a1), "f"(b));
 }
+// (d0, d1) = (a0, a1) + (c, c)
+__device__ __forceinline__ void addc2(float& d0, float& d1, float a0, float a1, float c) {
+  asm("{\n"
+      ".reg .b64 ra, rc;\n"
+      "mov.b64 ra, {%2, %3};\n"
+      "mov.b64 rc, {%4, %4};\n"
+      "add.rn.f32x2 ra, ra, rc;\n"
+      "mov.b64 {%0, %1}, ra;\n"
+      "}\n"
+      : "=f"(d0), "=f"(d1)
+      : "f"(a0), "f"(a1), "f"(c));
+}
+// (d0, d1) = (a0, a1) - (b0, b1)
+__device__ __forceinline__ void sub2(float& d0, float& d1, float a0, float a1, float b0, float b1) {
+  asm("{\n"
+      ".reg .b64 ra, rb;\n"
+      "mov.b64 ra, {%2, %3};\n"
+      "mov.b64 rb, {%4, %5};\n"
+      "sub.rn.f32x2 ra, ra, rb;\n"
+      "mov.b64 {%0, %1}, ra;\n"
+      "}\n"
+      : "=f"(d0), "=f"(d1)
+      : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
+// (d0, d1) = (a0, a1) * (b0, b1) + (c, c)
+__device__ __forceinline__ void fma2_pc(float& d0, float& d1, float a0, float a1, float b0, float b1, float c) {
+  asm("{\n"
+      ".reg .b64 ra, rb, rc;\n"
+      "mov.b64 ra, {%2, %3};\n"
+      "mov.b64 rb, {%4, %5};\n"
+      "mov.b64 rc, {%6, %6};\n"
+      "fma.rn.f32x2 ra, ra, rb, rc;\n"
+      "mov.b64 {%0, %1}, ra;\n"
+      "}\n"
+      : "=f"(d0), "=f"(d1)
+      : "f"(a0), "f"(a1), "f"(b0), "f"(b1), "f"(c));
+}
+// x << n as a funnel shift, which ptxas keeps on the ALU pipe (a plain shift becomes IMAD.SHL on the FMA pipe)
+__device__ __forceinline__ uint32_t shl_alu(uint32_t x, int n) {
+  uint32_t r;
+  asm("shf.l.wrap.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(0), "r"(x), "r"(n));
+  return r;
+}
 __device__ __forceinline__ float max3(float a, float b, float c) {
   float d;
   asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
