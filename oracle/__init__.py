@@ -17,7 +17,9 @@ visible key, P4 placement invariance, P5 suspend/resume identity, P6 reduction t
 torch SDPA, P7 chunked == monolithic, P8 batch-composition invariance, P9 softmax
 invariants + LSE merge, P10 window equivalence + page-count closed forms, P11
 hand-worked allocator trace (tests/golden/tiny_allocator_trace.txt), P12 distribution
-sanity.  Parity unpinned: none.
+sanity; migration (O4, `OraclePool.migrate_to`): M1 hand-worked id trace
+(tests/golden/migration_trace.txt), M2 == suspend + transplant + resume, M3 round trip and
+attention invariance, M4 conservation.  Parity unpinned: none.
 """
 from .pool import OraclePool, OracleError, INVALID, STATE, NO_PAGES, NO_HOST, CAPACITY, RESIDENT, SUSPENDED
 from .attention import chunk_attention, attention_rows

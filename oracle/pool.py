@@ -101,6 +101,39 @@ class OraclePool:
         s.host = None
         s.state = RESIDENT
 
+    # ---- GPU-GPU migration (O4; "migrates only the corresponding per-session state region";
+    #      :265 consistency protocol (i) freeze at a chunk boundary, (ii) target fetches and verifies that the
+    #      buffers are installed, (iii) ownership flips only after the transfer) ---------------------------
+    def migrate_to(self, sid, dst):
+        """Move RESIDENT session `sid` of this pool (the source worker) to pool `dst` (the target worker).
+        Reading R22 (the paper fixes neither ids nor page order): the target installs the session exactly as
+        a resume would - lowest unused id, |PT| pages popped from the FRONT of its free list, whole pages of
+        every layer copied in logical order (R11), same (P, o); the source then releases the session exactly
+        as a close would - its page ids go to the BACK of its free list in logical order and the id becomes
+        reusable.  All-or-nothing: every check comes before any change to either pool.  Returns the new id."""
+        s = self._get(sid)
+        if dst is self:
+            raise OracleError(INVALID, "migration to the same pool")
+        if (self.NL, self.H, self.D, self.B, self.T, self.W) != (dst.NL, dst.H, dst.D, dst.B, dst.T, dst.W):
+            raise OracleError(INVALID, "pools differ in geometry")
+        if s.state != RESIDENT:
+            raise OracleError(STATE, "migration of a non-resident session")   # (i): only a live, frozen state moves
+        new_sid = next((i for i in range(dst.max_sessions) if i not in dst.sessions), None)
+        if new_sid is None:
+            raise OracleError(CAPACITY, "no free session id on the target")
+        if len(s.PT) > len(dst.free):
+            raise OracleError(NO_PAGES, "target has too few free pages")
+        t = _Session()
+        t.P, t.o = s.P, s.o
+        t.PT = [dst.free.popleft() for _ in range(len(s.PT))]
+        for a, b in zip(s.PT, t.PT):                   # (ii) fetch: page by page, logical order, every layer
+            dst.K[:, b] = self.K[:, a]
+            dst.V[:, b] = self.V[:, a]
+        dst.sessions[new_sid] = t                      # (iii) ownership: installed on the target ...
+        self.free.extend(s.PT)                         # ... released on the source
+        del self.sessions[sid]
+        return new_sid
+
     # ---- append + window roll (O2; PAPER.md:66 (iii)) --------------------------------------------
     def append(self, layer, sids, chunk_frames, kn, vn, commit=True):
         """kn, vn: uint16 bf16 bits [sum C_s, H, D], sessions concatenated in `sids` order (R15)."""
