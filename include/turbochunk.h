@@ -190,6 +190,29 @@ int ts_session_resume(ts_pool* pool, int32_t sid);
 /* Host-blocks until all side-stream work enqueued so far has completed. */
 int ts_offload_sync(ts_pool* pool);
 
+/*
+ * PAPER.md:263 §6.1 "GPU-GPU state migration": move an active session from one worker (pool) to another by moving
+ * only its per-session state region; "the target worker can then fetch the registered state buffers from the source
+ * worker through ... one-sided GPU memory access and install them into its local session table".
+ * PAPER.md:265 "migration consistency": only at chunk boundaries; (i) the source completes the current chunk update
+ * and freezes the state, (ii) the target fetches it and verifies that the buffers are installed, (iii) ownership is
+ * updated only after the transfer completes.
+ * Reading R22 (the paper fixes neither ids nor page order): the target installs the session as a resume would -
+ * lowest free id (returned in *sid_out), |PT| pages popped from the FRONT of its free list, whole pages of every
+ * layer in logical order (R11), same (P, o), RESIDENT; the source releases it as a close would - page ids to the BACK
+ * of its free list in logical order, id reusable.
+ *   src, dst : two pools of identical geometry (NL, H, D, B, T, W), on the same device or on two devices of this
+ *              process with peer access (the fetch is ONE kernel on the target's device and side stream that reads
+ *              the source slab through the peer mapping: NVLink loads, no host staging, no copy-engine call per page).
+ *   sid      : RESIDENT session of src (a SUSPENDED one is TS_ERR_STATE: resume it where it should live instead).
+ * Ordering, all stream-side: the fetch starts after the compute work already enqueued on the session at the source
+ * (i); compute calls on the new session wait for the fetch (ii); the source's pages are not handed to a later writer
+ * before the fetch has completed (iii).  The host tables of both pools change at call time.
+ * Errors (nothing changes): TS_ERR_STATE (sid closed or not RESIDENT), TS_ERR_INVALID (src == dst, geometry differs),
+ * TS_ERR_CAPACITY (no free id on dst), TS_ERR_NO_PAGES (dst free list too short), TS_ERR_CUDA (no peer access).
+ */
+int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out);
+
 /* Introspection (parity is taken on these, never on raw slabs: the physical layout is private). */
 int ts_session_info(ts_pool* pool, int32_t sid, ts_session_info_t* out);
 /* Copies up to `cap` page ids (logical order) to `out` (host); *n_out = |PT|. */

@@ -19,7 +19,7 @@ TS_COMMIT = 1
 EXPORTED_SYMBOLS = [
     "ts_pool_page_bytes", "ts_pool_slab_bytes", "ts_pool_create", "ts_pool_destroy", "ts_session_open",
     "ts_session_close", "ts_chunk_attention", "ts_kv_append", "ts_chunk_step", "ts_chunk_step_host", "ts_session_suspend",
-    "ts_session_resume", "ts_offload_sync", "ts_session_info", "ts_session_page_table", "ts_gather_kv",
+    "ts_session_resume", "ts_session_migrate", "ts_offload_sync", "ts_session_info", "ts_session_page_table", "ts_gather_kv",
     "ts_pool_free_list", "ts_pool_stats", "ts_pool_side_stream", "ts_pool_launch_count", "ts_strerror",
     "ts_last_cuda_error", "ts_version",
 ]
@@ -65,6 +65,7 @@ def _load():
     L.ts_chunk_step_host.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, P, P, C.c_float, C.c_uint32, P]
     L.ts_session_suspend.argtypes = [P, C.c_int32]
     L.ts_session_resume.argtypes = [P, C.c_int32]
+    L.ts_session_migrate.argtypes = [P, C.c_int32, P, I32P]
     L.ts_offload_sync.argtypes = [P]
     L.ts_session_info.argtypes = [P, C.c_int32, C.POINTER(ts_session_info_t)]
     L.ts_session_page_table.argtypes = [P, C.c_int32, I32P, C.c_int32, I32P]
@@ -196,6 +197,12 @@ class TurboChunkPool:
 
     def ts_session_resume(self, sid):
         _check(lib.ts_session_resume(self._h, sid), "ts_session_resume")
+
+    def ts_session_migrate(self, sid, dst):
+        """Move RESIDENT session `sid` of this pool to pool `dst`; returns its id there."""
+        new = C.c_int32(-1)
+        _check(lib.ts_session_migrate(self._h, sid, dst._h, C.byref(new)), "ts_session_migrate")
+        return new.value
 
     def ts_offload_sync(self):
         _check(lib.ts_offload_sync(self._h), "ts_offload_sync")

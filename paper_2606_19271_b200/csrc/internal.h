@@ -62,6 +62,15 @@ struct CopyParams {
   uint8_t* dst_v;
 };
 
+struct PullParams {          // migration fetch: whole pages, source slab -> target slab
+  const uint8_t* src_slab;   // may be peer memory (another device of this process)
+  uint8_t* dst_slab;
+  const int32_t* pairs;      // device [n_pages][2]: (source page id, target page id), logical order
+  int32_t n_pages;
+  int32_t vec_per_page;      // page bytes / 16
+  int64_t page_stride;       // bytes per page, same in both slabs (identical geometry)
+};
+
 constexpr int kFeedRing = 16;   // entries of a cluster's item-feed ring
 
 struct AttnParams {
@@ -87,6 +96,7 @@ struct AttnParams {
 cudaError_t launch_attention(const AttnParams& p, int head_dim, int grid, cudaStream_t stream);
 cudaError_t launch_append(const CopyParams& p, int sm_count, cudaStream_t stream);
 cudaError_t launch_gather(const CopyParams& p, int sm_count, cudaStream_t stream);
+cudaError_t launch_page_pull(const PullParams& p, int sm_count, cudaStream_t stream);
 int attention_smem_bytes(int head_dim);
 
 }  // namespace tc

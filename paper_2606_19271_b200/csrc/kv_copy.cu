@@ -67,6 +67,40 @@ __global__ void __launch_bounds__(kCopyThreads) kv_gather_kernel(const CopyParam
   }
 }
 
+// Migration fetch (the TARGET worker fetches the state buffers from the source through one-sided GPU
+// memory access).  blockIdx.y = page of the session (logical order), blockIdx.x strides over the page's 16-byte
+// vectors; kPullUnroll independent 128-bit loads in flight per thread (the source may sit behind NVLink).  On one
+// device it is HBM-bound: algorithmic bytes = 2 * n_pages * page bytes.
+constexpr int kPullUnroll = 8;
+
+__global__ void __launch_bounds__(kCopyThreads) page_pull_kernel(const PullParams p) {
+  const int32_t sp = p.pairs[2 * blockIdx.y], dp = p.pairs[2 * blockIdx.y + 1];
+  const uint8_t* src = p.src_slab + (int64_t)sp * p.page_stride;
+  uint8_t* dst = p.dst_slab + (int64_t)dp * p.page_stride;
+  const int stride = gridDim.x * kCopyThreads;
+  for (int e0 = blockIdx.x * kCopyThreads + threadIdx.x; e0 < p.vec_per_page; e0 += stride * kPullUnroll) {
+    uint4 r[kPullUnroll];
+#pragma unroll
+    for (int u = 0; u < kPullUnroll; ++u) {
+      const int e = e0 + u * stride;
+      if (e < p.vec_per_page) r[u] = ld_stream(src + (int64_t)e * 16);
+    }
+#pragma unroll
+    for (int u = 0; u < kPullUnroll; ++u) {
+      const int e = e0 + u * stride;
+      if (e < p.vec_per_page) *reinterpret_cast<uint4*>(dst + (int64_t)e * 16) = r[u];
+    }
+  }
+}
+
+cudaError_t launch_page_pull(const PullParams& p, int sm_count, cudaStream_t stream) {
+  const int want = (p.vec_per_page + kCopyThreads * kPullUnroll - 1) / (kCopyThreads * kPullUnroll);
+  const int cap = (sm_count * 8 + p.n_pages - 1) / p.n_pages;   // 8 resident CTAs of 256 threads per SM
+  const int gx = want < cap ? want : cap;
+  page_pull_kernel<<<dim3((unsigned)(gx < 1 ? 1 : gx), (unsigned)p.n_pages, 1), kCopyThreads, 0, stream>>>(p);
+  return cudaGetLastError();
+}
+
 static dim3 copy_grid(const CopyParams& p, int sm_count, int64_t max_vecs_per_sess) {
   // enough CTAs to fill the machine (8 resident CTAs of 256 threads per SM), split evenly over sessions
   int64_t want = (max_vecs_per_sess + (int64_t)kCopyThreads * kCopyUnroll - 1) / ((int64_t)kCopyThreads * kCopyUnroll);

@@ -1045,6 +1045,94 @@ int ts_session_resume(ts_pool* pool, int32_t sid) {
   return TS_OK;
 }
 
+// --------------------------------------------------------------------------------------------- migration
+int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out) {
+  if (src == nullptr || dst == nullptr || sid_out == nullptr) return TS_ERR_INVALID;
+  if (sid < 0 || sid >= src->cfg.max_sessions || src->sess[sid].state == TS_SESSION_CLOSED) return TS_ERR_STATE;
+  const ts_pool_config &a = src->cfg, &b = dst->cfg;
+  if (src == dst) return TS_ERR_INVALID;
+  if (a.n_layers != b.n_layers || a.n_heads != b.n_heads || a.head_dim != b.head_dim || a.page_tokens != b.page_tokens ||
+      a.frame_tokens != b.frame_tokens || a.window_frames != b.window_frames)
+    return TS_ERR_INVALID;
+  Session& s = src->sess[sid];
+  if (s.state != TS_SESSION_RESIDENT) return TS_ERR_STATE;   // (i): only a live, frozen state moves
+  int new_sid = -1;
+  for (int i = 0; i < b.max_sessions && new_sid < 0; ++i)
+    if (dst->sess[i].state == TS_SESSION_CLOSED) new_sid = i;
+  if (new_sid < 0) return TS_ERR_CAPACITY;
+  const size_t n = s.pt.size();
+  if (n > dst->free_q.size()) return TS_ERR_NO_PAGES;
+  TS_CUDA(cudaSetDevice(b.device));
+  if (a.device != b.device) {   // one-sided access: the target maps the source's memory ("registers")
+    int can = 0;
+    TS_CUDA(cudaDeviceCanAccessPeer(&can, b.device, a.device));
+    if (!can) {
+      g_last_cuda_error = "no peer access from the target device to the source device";
+      return TS_ERR_CUDA;
+    }
+    const cudaError_t e = cudaDeviceEnablePeerAccess(a.device, 0);
+    if (e == cudaErrorPeerAccessAlreadyEnabled) cudaGetLastError();
+    else TS_CUDA(e);
+  }
+  Staging* st = nullptr;
+  if (n > 0) {
+    const int rc = acquire_staging(dst, n * 8, &st);
+    if (rc != TS_OK) return rc;
+  }
+  // ---- nothing can fail for a reason of ours from here on: install on the target (as a resume would)
+  Session& t = dst->sess[new_sid];
+  t = Session();
+  t.P = s.P;
+  t.o = s.o;
+  uint64_t wait_compute = 0;
+  for (size_t i = 0; i < n; ++i) {
+    const int32_t pg = dst->free_q.front();
+    dst->free_q.pop_front();
+    wait_compute = std::max(wait_compute, dst->page_compute_seq[pg]);   // readers of the page's previous owner
+    t.pt.push_back(pg);                                                 // (copies out of it are on this side stream)
+  }
+  uint64_t seq_src = s.side_seq;
+  if (n > 0) {
+    int32_t* pairs = reinterpret_cast<int32_t*>(st->h);
+    for (size_t i = 0; i < n; ++i) {
+      pairs[2 * i] = s.pt[i];
+      pairs[2 * i + 1] = t.pt[i];
+    }
+    // (i) chunk boundary: after the compute work already enqueued on the session at the source, and after a resume
+    // of it that may still be copying in
+    TS_CUDA(src->tl_compute.wait(dst->side, s.compute_seq));
+    TS_CUDA(src->tl_side.wait(dst->side, s.side_seq));
+    TS_CUDA(dst->tl_compute.wait(dst->side, wait_compute));
+    TS_CUDA(cudaMemcpyAsync(st->d, st->h, n * 8, cudaMemcpyHostToDevice, dst->side));
+    PullParams p;
+    p.src_slab = src->slab;
+    p.dst_slab = dst->slab;
+    p.pairs = reinterpret_cast<const int32_t*>(st->d);
+    p.n_pages = (int32_t)n;
+    p.vec_per_page = (int32_t)(dst->page_bytes / 16);
+    p.page_stride = dst->page_bytes;
+    TS_CUDA(launch_page_pull(p, dst->sm_count, dst->side));   // (ii) the target fetches
+    ++dst->launches;
+    TS_CUDA(cudaEventRecord(st->ev, dst->side));
+    st->in_flight = true;
+    t.side_seq = dst->tl_side.record(dst->side);              // compute calls on the new session wait for this
+    // (iii) the source's pages may be rewritten only after the fetch: mark that point on the source's side timeline
+    TS_CUDA(dst->tl_side.wait(src->side, t.side_seq));
+    TS_CUDA(cudaSetDevice(a.device));
+    seq_src = src->tl_side.record(src->side);
+  }
+  t.ver = ++dst->ver_seq;
+  t.state = TS_SESSION_RESIDENT;
+  for (int32_t pg : s.pt) {                                   // release on the source (as a close would)
+    src->page_side_seq[pg] = seq_src;
+    src->page_compute_seq[pg] = s.compute_seq;
+    src->free_q.push_back(pg);
+  }
+  s = Session();
+  *sid_out = new_sid;
+  return TS_OK;
+}
+
 int ts_offload_sync(ts_pool* pool) {
   if (pool == nullptr) return TS_ERR_INVALID;
   TS_CUDA(cudaSetDevice(pool->cfg.device));
