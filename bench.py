@@ -323,6 +323,7 @@ def main():
 
     # ---- offload leg (side stream, timed alone): suspend / resume of a full-window session
     off = measure_offload(wl)
+    mig = measure_migration(wl, peaks["hbm_gbs"])
 
     # ---- end to end through ts_chunk_step_host with pinned host buffers
     hq, hk, hv = (t.cpu().pin_memory() for t in (wl["q"], wl["k"], wl["v"]))
@@ -371,6 +372,7 @@ def main():
                    "peak": peaks["hbm_gbs"], "unit": "GB/s",
                    "frac": round(append_bytes / (append_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], 4)},
         "offload": off,
+        "migrate": mig,
         "e2e": {"value": round(flops_step * args.steps * world / (e2e_ms_all * 1e-3) / 1e12, 2), "unit": UNIT,
                 "ms_per_step": round(e2e_ms_all / args.steps, 4), "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "api": "ts_chunk_step_host (pinned host Q/K/V/O)"},
@@ -445,6 +447,51 @@ def measure_offload(wl):
     res["peak_kind"] = "one pinned cudaMemcpyAsync of the same bytes, same run"
     pool.close()
     return res
+
+
+def measure_migration(wl, hbm_peak):
+    """ts_session_migrate of a full-window (21-frame) session between two pools, ping-pong, 8 moves enqueued back to
+    back behind a blocker copy (so that the host's enqueue time is not in the events).  Both pools sit on this one GPU,
+    where the fetch kernel is HBM-bound (read + write of the session's pages); between two GPUs the same kernel reads
+    the source slab over NVLink - not measurable on a 1-GPU box."""
+    import torch
+    from synth.draw import draw_bits_torch
+    from paper_2606_19271_b200 import TS_COMMIT, TurboChunkPool
+    sh = wl["w"].shape
+    T, H, D = sh.frame_tokens, sh.n_heads, sh.head_dim
+    dev = wl["q"].device
+    pools = [TurboChunkPool(1, H, D, sh.page_tokens, 160, T, sh.window_frames, 2, device=dev.index) for _ in range(2)]
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(98)
+    sid = pools[0].ts_session_open()
+    for _ in range(7):
+        kk = draw_bits_torch(gen, 3 * T, H, D, dev)
+        pools[0].ts_kv_append(0, [sid], [3], kk, kk, TS_COMMIT)
+    n_pages = pools[0].ts_session_info(sid)["n_pages"]
+    nbytes = n_pages * pools[0].page_bytes
+    blocker_src = torch.empty(1 << 30, dtype=torch.uint8, device=dev)
+    blocker_dst = torch.empty_like(blocker_src)
+    n_moves, best = 8, 1e9
+    torch.cuda.synchronize()
+    for _ in range(3):
+        first = pools[1].side_stream
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(first):
+            blocker_dst.copy_(blocker_src, non_blocking=True)
+        e0.record(first)
+        for i in range(n_moves):
+            src, dst = pools[i & 1], pools[(i & 1) ^ 1]
+            sid = src.ts_session_migrate(sid, dst)
+        e1.record(pools[(n_moves - 1) & 1 ^ 1].side_stream)
+        torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1) / n_moves)
+    gbs = 2 * nbytes / (best * 1e-3) / 1e9
+    for p in pools:
+        p.close()
+    return {"bound": "hbm", "kernel": "page_pull_kernel", "bytes_moved": int(nbytes), "pages": int(n_pages),
+            "algorithmic_bytes_per_launch": int(2 * nbytes), "ms_per_move": round(best, 4), "achieved": round(gbs, 1),
+            "peak": hbm_peak, "unit": "GB/s", "frac": round(gbs / hbm_peak, 4),
+            "note": "both pools on this GPU (read + write in HBM); across GPUs the fetch reads over NVLink"}
 
 
 def run_reference(args):
