@@ -100,7 +100,8 @@ struct Staging {      // pinned host + device buffer pair for per-call schedule 
   uint8_t* h = nullptr;
   uint8_t* d = nullptr;
   size_t cap = 0;
-  cudaEvent_t ev = nullptr;
+  cudaEvent_t ev = nullptr;      // recorded on the consumer's stream after the kernel that reads `d`
+  cudaEvent_t ev_up = nullptr;   // recorded on the pool's upload stream after the H2D of the block
   bool in_flight = false;
 };
 
@@ -131,6 +132,7 @@ struct ts_pool {
   static constexpr int kRing = 8;
   Staging ring[kRing];
   int ring_next = 0;
+  cudaStream_t up_s = nullptr;             // upload stream of the per-call schedule / descriptor blocks
   uint8_t* stage_dev = nullptr;            // ts_chunk_step_host: two device staging sets for q,k,v,out
   cudaStream_t h2d_s = nullptr, d2h_s = nullptr;   // ... its copy streams (input of step t+1 overlaps step t)
   cudaEvent_t ev_in = nullptr, ev_attn = nullptr, ev_out = nullptr, ev_free[2] = {nullptr, nullptr};
@@ -165,6 +167,7 @@ static int acquire_staging(ts_pool* pool, size_t bytes, Staging** out) {
   Staging& s = pool->ring[pool->ring_next];
   pool->ring_next = (pool->ring_next + 1) % ts_pool::kRing;
   if (s.ev == nullptr) TS_CUDA(cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming));
+  if (s.ev_up == nullptr) TS_CUDA(cudaEventCreateWithFlags(&s.ev_up, cudaEventDisableTiming));
   if (s.in_flight) {
     TS_CUDA(cudaEventSynchronize(s.ev));   // normally long done: the ring is 8 calls deep
     s.in_flight = false;
@@ -180,6 +183,17 @@ static int acquire_staging(ts_pool* pool, size_t bytes, Staging** out) {
     s.cap = cap;
   }
   *out = &s;
+  return TS_OK;
+}
+
+// The per-call descriptor block does not depend on anything the caller's stream is doing: it is uploaded on the pool's
+// own stream, so that the copy runs under the previous kernel instead of between two kernels of the caller's stream,
+// which only waits for the (normally long complete) upload event.
+static int upload_staging(ts_pool* pool, Staging* st, size_t bytes, cudaStream_t consumer) {
+  if (pool->up_s == nullptr) TS_CUDA(cudaStreamCreateWithFlags(&pool->up_s, cudaStreamNonBlocking));
+  TS_CUDA(cudaMemcpyAsync(st->d, st->h, bytes, cudaMemcpyHostToDevice, pool->up_s));
+  TS_CUDA(cudaEventRecord(st->ev_up, pool->up_s));
+  TS_CUDA(cudaStreamWaitEvent(consumer, st->ev_up, 0));
   return TS_OK;
 }
 
@@ -286,7 +300,9 @@ int ts_pool_destroy(ts_pool* pool) {
     if (s.h) cudaFreeHost(s.h);
     if (s.d) cudaFree(s.d);
     if (s.ev) cudaEventDestroy(s.ev);
+    if (s.ev_up) cudaEventDestroy(s.ev_up);
   }
+  if (pool->up_s) cudaStreamDestroy(pool->up_s);
   if (pool->stage_dev) cudaFree(pool->stage_dev);
   if (pool->h2d_s) cudaStreamDestroy(pool->h2d_s);
   if (pool->d2h_s) cudaStreamDestroy(pool->d2h_s);
@@ -706,7 +722,8 @@ static int attention_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t
     TS_CUDA(pool->tl_compute.wait(stream, fused->wait_compute));
   }
 
-  TS_CUDA(cudaMemcpyAsync(st->d, st->h, L.bytes, cudaMemcpyHostToDevice, stream));
+  rc = upload_staging(pool, st, L.bytes, stream);
+  if (rc != TS_OK) return rc;
   AttnParams p;
   memset(&p.copy, 0, sizeof(p.copy));
   if (fused) {
@@ -850,7 +867,8 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, c
   }
   TS_CUDA(pool->tl_side.wait(stream, wait_side));
   TS_CUDA(pool->tl_compute.wait(stream, wait_compute));
-  TS_CUDA(cudaMemcpyAsync(st->d, st->h, bytes, cudaMemcpyHostToDevice, stream));
+  rc = upload_staging(pool, st, bytes, stream);
+  if (rc != TS_OK) return rc;
   CopyParams p;
   memset(&p, 0, sizeof(p));
   p.sess = reinterpret_cast<const CopySess*>(st->d + off_sess);
@@ -963,7 +981,8 @@ int ts_gather_kv(ts_pool* pool, int32_t layer, int32_t sid, void* k_out, void* v
   cs->pad0 = cs->pad1 = 0;
   std::copy(s.pt.begin(), s.pt.end(), reinterpret_cast<int32_t*>(st->h + off_pt));
   TS_CUDA(pool->tl_side.wait(stream, s.side_seq));
-  TS_CUDA(cudaMemcpyAsync(st->d, st->h, bytes, cudaMemcpyHostToDevice, stream));
+  rc = upload_staging(pool, st, bytes, stream);
+  if (rc != TS_OK) return rc;
   CopyParams p;
   memset(&p, 0, sizeof(p));
   p.sess = reinterpret_cast<const CopySess*>(st->d);
