@@ -23,6 +23,7 @@ attention invariance, M4 conservation.  Parity unpinned: none.
 """
 from .pool import OraclePool, OracleError, INVALID, STATE, NO_PAGES, NO_HOST, CAPACITY, RESIDENT, SUSPENDED
 from .attention import chunk_attention, attention_rows
+from .scheduler import SchedulerOracle
 
 __all__ = ["OraclePool", "OracleError", "INVALID", "STATE", "NO_PAGES", "NO_HOST", "CAPACITY",
-           "RESIDENT", "SUSPENDED", "chunk_attention", "attention_rows"]
+           "RESIDENT", "SUSPENDED", "chunk_attention", "attention_rows", "SchedulerOracle"]
