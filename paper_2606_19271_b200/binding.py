@@ -22,6 +22,7 @@ EXPORTED_SYMBOLS = [
     "ts_session_resume", "ts_session_migrate", "ts_offload_sync", "ts_session_info", "ts_session_page_table", "ts_gather_kv",
     "ts_pool_free_list", "ts_pool_stats", "ts_pool_side_stream", "ts_pool_launch_count", "ts_strerror",
     "ts_last_cuda_error", "ts_version",
+    "ts_sched_create", "ts_sched_destroy", "ts_sched_event", "ts_sched_moves", "ts_sched_alive",
 ]
 
 
@@ -42,6 +43,19 @@ class ts_pool_stats_t(C.Structure):
     _fields_ = [("free_pages", C.c_int32), ("resident", C.c_int32), ("suspended", C.c_int32),
                 ("host_pages_used", C.c_int32), ("host_pages_cap", C.c_int32), ("reserved", C.c_int32),
                 ("page_bytes", C.c_int64)]
+
+
+class ts_sched_config(C.Structure):
+    _fields_ = [("K", C.c_int32), ("M_max", C.c_int32), ("M0", C.c_int32), ("vol_window", C.c_int32),
+                ("rho_hat", C.c_double), ("delta", C.c_double), ("eta", C.c_double), ("kappa_alpha", C.c_double),
+                ("kappa_beta", C.c_double), ("l_hat", C.POINTER(C.c_double)), ("n_levels", C.c_int32),
+                ("reserved", C.c_int32), ("vol_bounds", C.POINTER(C.c_double)), ("vol_rho", C.POINTER(C.c_double))]
+
+
+class ts_sched_result(C.Structure):
+    _fields_ = [("M", C.c_int32), ("n_migrations", C.c_int32), ("n_moves", C.c_int32), ("n_unplaced", C.c_int32),
+                ("n_req", C.c_int32), ("reserved", C.c_int32), ("rho_max", C.c_double), ("L", C.c_double),
+                ("rho_hat", C.c_double), ("sigma", C.c_double)]
 
 
 def _load():
@@ -76,6 +90,12 @@ def _load():
     L.ts_pool_side_stream.argtypes = [P]
     L.ts_pool_launch_count.restype = C.c_int64
     L.ts_pool_launch_count.argtypes = [P]
+    DP = C.POINTER(C.c_double)
+    L.ts_sched_create.argtypes = [C.POINTER(ts_sched_config), C.POINTER(P)]
+    L.ts_sched_destroy.argtypes = [P]
+    L.ts_sched_event.argtypes = [P, C.c_int32, I32P, I32P, DP, I32P, C.POINTER(ts_sched_result)]
+    L.ts_sched_moves.argtypes = [P, C.c_int32, I32P, I32P, I32P, C.c_int32, I32P]
+    L.ts_sched_alive.argtypes = [P, I32P]
     L.ts_strerror.restype = C.c_char_p
     L.ts_strerror.argtypes = [C.c_int]
     L.ts_last_cuda_error.restype = C.c_char_p
@@ -247,3 +267,59 @@ class TurboChunkPool:
     @property
     def side_stream(self):
         return self._side
+
+
+class TurboSched:
+    """ctypes view of include/turbochunk_sched.h (the closed-loop scheduler, §5.2).  Host code only."""
+
+    def __init__(self, K, M_max, M0, l_hat, rho_hat=0.7, delta=0.1, eta=0.0, kappa_alpha=0.0, kappa_beta=0.0,
+                 vol_window=0, vol_bounds=(), vol_rho=()):
+        cfg = ts_sched_config()
+        cfg.K, cfg.M_max, cfg.M0, cfg.vol_window = K, M_max, M0, vol_window
+        cfg.rho_hat, cfg.delta, cfg.eta, cfg.kappa_alpha, cfg.kappa_beta = rho_hat, delta, eta, kappa_alpha, kappa_beta
+        self._l_hat = (C.c_double * len(l_hat))(*[float(x) for x in l_hat])
+        cfg.l_hat = C.cast(self._l_hat, C.POINTER(C.c_double))
+        cfg.n_levels = len(vol_rho)
+        self._vb = (C.c_double * max(1, len(vol_bounds)))(*[float(x) for x in vol_bounds])
+        self._vr = (C.c_double * max(1, len(vol_rho)))(*[float(x) for x in vol_rho])
+        cfg.vol_bounds = C.cast(self._vb, C.POINTER(C.c_double))
+        cfg.vol_rho = C.cast(self._vr, C.POINTER(C.c_double))
+        if len(l_hat) != K + 1 or (vol_window and len(vol_bounds) != len(vol_rho) - 1):
+            raise TurboChunkError(TS_ERR_INVALID, "ts_sched_create")
+        self.M_max = M_max
+        h = C.c_void_p()
+        _check(lib.ts_sched_create(C.byref(cfg), C.byref(h)), "ts_sched_create")
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib.ts_sched_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _moves(self, which):
+        n = C.c_int32(0)
+        _check(lib.ts_sched_moves(self._h, which, None, None, None, 0, C.byref(n)), "ts_sched_moves")
+        a, b, c = ((C.c_int32 * max(1, n.value))() for _ in range(3))
+        _check(lib.ts_sched_moves(self._h, which, a, b, c, n.value, C.byref(n)), "ts_sched_moves")
+        return [(a[i], b[i], c[i]) for i in range(n.value)]
+
+    def ts_sched_event(self, sessions):
+        """sessions: list of (session id, alpha, state_mb) in event order; returns the decision of Algorithm 1."""
+        n = len(sessions)
+        ids = _i32([s[0] for s in sessions])
+        act = _i32([s[1] for s in sessions])
+        mb = (C.c_double * max(1, n))(*[float(s[2]) for s in sessions])
+        phi = (C.c_int32 * max(1, n))()
+        res = ts_sched_result()
+        _check(lib.ts_sched_event(self._h, n, ids, act, mb, phi, C.byref(res)), "ts_sched_event")
+        alive = (C.c_int32 * self.M_max)()
+        _check(lib.ts_sched_alive(self._h, alive), "ts_sched_alive")
+        return {"M": res.M, "alive": [j for j in range(self.M_max) if alive[j]], "rho_max": res.rho_max, "L": res.L,
+                "phi": {sessions[i][0]: phi[i] for i in range(n)}, "migrations": self._moves(0), "moves": self._moves(1),
+                "n_unplaced": res.n_unplaced, "rho_hat": res.rho_hat, "sigma": res.sigma, "n_req": res.n_req}

@@ -6,8 +6,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libturbochunk.so")
-SOURCES = ["pool.cu", "kv_copy.cu", "attention_sm100.cu"]
-HEADERS = ["internal.h", "ptx.cuh", "kv_copy.cuh", os.path.join("..", "..", "include", "turbochunk.h")]
+SOURCES = ["pool.cu", "kv_copy.cu", "attention_sm100.cu", "sched.cpp"]
+HEADERS = ["internal.h", "ptx.cuh", "kv_copy.cuh", os.path.join("..", "..", "include", "turbochunk.h"),
+           os.path.join("..", "..", "include", "turbochunk_sched.h")]
 
 
 def _stale():
@@ -23,7 +24,7 @@ def build(force=False, verbose=False):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-           "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v", "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+           "-Xcompiler", "-fPIC", "-Xcompiler", "-ffp-contract=off", "-shared", "-Xptxas", "-v", "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     log = res.stdout + res.stderr
     with open(os.path.join(HERE, "build.log"), "w") as f:
