@@ -616,3 +616,49 @@ def test_chunk_step_fused_equals_sequence():
         dq2.g.ts_chunk_step(0, [s0], [3], bits_to_dev(q), bits_to_dev(k), bits_to_dev(v), torch.empty(3 * T, 3, 128, dtype=torch.bfloat16, device="cuda"), None, 0.1, TS_COMMIT)
     assert e.value.code == tc.TS_ERR_NO_PAGES
     dq2.check_state([s0])
+
+
+# ---- the lazy-rescale path and the split-tile merge under large score jumps (N(0,1) inputs almost never take them) -----------
+@pytest.mark.parametrize("pattern", ["ramp_up", "ramp_down", "spikes", "masked_spike"])
+@pytest.mark.parametrize("page_tokens", [64, 256])
+def test_lazy_rescale_and_outliers(pattern, page_tokens):
+    """Scores that jump by far more than the rescale threshold (2^8) from tile to tile, in both directions, inside either
+    64-key half of a tile, in the chunk, and behind the frame mask: every rescale of O in TMEM, the (m, l) merge of a split
+    lone tile and the mask must hold against the fp64 oracle."""
+    f32_to_bf16_bits = synth.f32_to_bf16_bits
+    T, H, D, prior, c = 160, 2, 128, 6, 2
+    shape = shape_of(n_heads=H, head_dim=D, page_tokens=page_tokens, frame_tokens=T, n_pages=64, window_frames=0)
+    rng = np.random.default_rng(len(pattern) * 37 + page_tokens)
+    dp = DualPool(shape, rng.permutation(shape.n_pages))
+    sid = dp.open()
+    Lp, C = prior * T, c * T
+    u = np.ones(D, dtype=np.float32) / np.sqrt(np.float32(D))
+    a = np.zeros(Lp + C, dtype=np.float32)                       # boost of key j along u
+    if pattern == "ramp_up":
+        a[:] = 0.125 * np.arange(Lp + C)                         # +5.6 nats per 128-key tile, logits up to ~56 nats
+    elif pattern == "ramp_down":
+        a[:] = 0.125 * np.arange(Lp + C)[::-1]
+    elif pattern == "spikes":
+        for j in (5, 100, 128 + 70, 3 * 128 + 64, 5 * 128 + 127, Lp - 1, Lp + 3, Lp + 130, Lp + T - 1):
+            a[j] = 150.0 + j % 7                                  # isolated keys ~50 nats above the rest
+    else:                                                         # a huge key in the chunk's SECOND frame: frame-0 queries
+        a[Lp + T + 17] = 400.0                                    # must not see it, frame-1 queries are dominated by it
+        a[Lp + 2 * T - 1] = 380.0
+    noise = lambda n: rng.standard_normal((n, H, D)).astype(np.float32) * 0.5
+    k_all = noise(Lp + C) + a[:, None, None] * u[None, None, :]
+    v_all = rng.standard_normal((Lp + C, H, D)).astype(np.float32)
+    q = noise(C) + 4.0 * u[None, None, :]
+    kb, vb, qb = f32_to_bf16_bits(k_all), f32_to_bf16_bits(v_all), f32_to_bf16_bits(q)
+    dp.feed_prior(sid, [kb[:Lp]], [vb[:Lp]])
+    o_gpu, o_ref = dp.attention(0, [sid], [c], qb, kb[Lp:], vb[Lp:], scale_of(shape))
+    if pattern == "masked_spike":
+        # frame-0 rows ignore the spike entirely; frame-1 rows are (almost) exactly v of the spike key
+        v_spike = synth.bf16_bits_to_f64(vb[Lp + T + 17])
+        assert np.abs(o_gpu[T:] - v_spike[None]).max() < 0.15     # the second, smaller spike keeps a weight of ~1 %
+        assert np.abs(o_gpu[:T] - v_spike[None]).max() > 0.5
+    # a second session in the same batch with plain N(0,1) inputs must be unaffected (isolation inside one launch)
+    other = dp.open()
+    dp.feed_prior(other, [draw(rng, 3 * T, shape)], [draw(rng, 3 * T, shape)])
+    q2, k2, v2 = (draw(rng, 3 * T, shape) for _ in range(3))
+    dp.attention(0, [other, sid], [3, c], np.concatenate([q2, qb]), np.concatenate([k2, kb[Lp:]]),
+                 np.concatenate([v2, vb[Lp:]]), scale_of(shape))
