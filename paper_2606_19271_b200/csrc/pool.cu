@@ -1136,8 +1136,8 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
     st->in_flight = true;
     t.side_seq = dst->tl_side.record(dst->side);              // compute calls on the new session wait for this
     // (iii) the source's pages may be rewritten only after the fetch: mark that point on the source's side timeline
-    TS_CUDA(dst->tl_side.wait(src->side, t.side_seq));
     TS_CUDA(cudaSetDevice(a.device));
+    TS_CUDA(dst->tl_side.wait(src->side, t.side_seq));
     seq_src = src->tl_side.record(src->side);
   }
   t.ver = ++dst->ver_seq;
