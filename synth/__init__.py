@@ -9,11 +9,11 @@ permutations, the churn event script).  Recipes: DESIGN.md §"Input recipe".
 from .bf16 import f32_to_bf16_bits, bf16_bits_to_f32, bf16_bits_to_f64
 from .configs import (PoolShape, SessionSpec, Workload, tiny, wan13b_single,
                       wan13b_batch, wan14b_batch, churn_script, attention_flops,
-                      attention_pairs, CONFIG_BUILDERS)
+                      attention_pairs, CONFIG_BUILDERS, sched_events)
 from .draw import draw_bits, draw_session_tensors
 
 __all__ = [
     "f32_to_bf16_bits", "bf16_bits_to_f32", "bf16_bits_to_f64", "PoolShape", "SessionSpec",
     "Workload", "tiny", "wan13b_single", "wan13b_batch", "wan14b_batch", "churn_script",
-    "attention_flops", "attention_pairs", "CONFIG_BUILDERS", "draw_bits", "draw_session_tensors",
+    "attention_flops", "attention_pairs", "CONFIG_BUILDERS", "sched_events", "draw_bits", "draw_session_tensors",
 ]

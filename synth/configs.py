@@ -165,3 +165,26 @@ def churn_script(seed=4, n_steps=200, cap=32, mean_off=4.0, mean_on=24.0, p_off_
         ev["mode_on"] = mode_on
         steps.append(ev)
     return steps
+
+
+def sched_events(seed, n_events, cap, p_on=0.05, p_off=0.10, mean_off=0.4, mean_on=3.0, p_leave=0.04, p_flip=0.15):
+    """Seeded event stream for the closed-loop scheduler (§5.1 "event-driven scheduling"): per event the list of
+    live sessions `(id, alpha, state size in MB)`.  Structure: bursty on/off arrivals (an off/on Markov chain modulating a
+    Poisson arrival count, the shape PAPER.md:36-38 describes), departures, active <-> idle flips; now and then the
+    sessions are listed in a shuffled order.  The paper's production traces are not available; this stands in for them."""
+    rng = np.random.default_rng(seed)
+    live, next_id, on = {}, 0, False
+    for _ in range(n_events):
+        on = (rng.random() < p_on) if not on else (rng.random() >= p_off)
+        for sid in list(live):
+            u = rng.random()
+            if u < p_leave:
+                del live[sid]
+            elif u < p_leave + p_flip:
+                live[sid] = (1 - live[sid][0], live[sid][1])
+        for _ in range(rng.poisson(mean_on if on else mean_off)):
+            if len(live) < cap:
+                live[next_id] = (1, float(rng.integers(30, 210)) + 0.25 * float(rng.integers(0, 4)))
+                next_id += 1
+        order = sorted(live) if rng.random() < 0.8 else [int(x) for x in rng.permutation(sorted(live))]
+        yield [(sid, live[sid][0], live[sid][1]) for sid in order]

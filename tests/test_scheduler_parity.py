@@ -5,6 +5,8 @@ order and must be bit-identical too.  Host code only: runs without a GPU."""
 import numpy as np
 import pytest
 
+import synth
+
 from oracle import SchedulerOracle
 
 LHAT5 = [0, 90, 174, 267, 350, 441]          # measured l_hat(n), DESIGN.md §7.2
@@ -19,24 +21,8 @@ def TurboSched():
     return TurboSched
 
 
-def event_stream(seed, n_events, cap, p_on=0.05, p_off=0.10, mean_off=0.4, mean_on=3.0, p_leave=0.04, p_flip=0.15):
-    """Bursty on/off arrivals (the structure of configs[4]'s churn: PAPER.md:36-38), departures, active <-> idle flips."""
-    rng = np.random.default_rng(seed)
-    live, next_id, on = {}, 0, False
-    for _ in range(n_events):
-        on = (rng.random() < p_on) if not on else (rng.random() >= p_off)
-        for sid in list(live):
-            u = rng.random()
-            if u < p_leave:
-                del live[sid]
-            elif u < p_leave + p_flip:
-                live[sid] = (1 - live[sid][0], live[sid][1])
-        for _ in range(rng.poisson(mean_on if on else mean_off)):
-            if len(live) < cap:
-                live[next_id] = (1, float(rng.integers(30, 210)) + 0.25 * float(rng.integers(0, 4)))
-                next_id += 1
-        order = sorted(live) if rng.random() < 0.8 else [int(x) for x in rng.permutation(sorted(live))]
-        yield [(sid, live[sid][0], live[sid][1]) for sid in order]
+def event_stream(seed, n_events, cap, **kw):
+    return synth.sched_events(seed, n_events, cap, **kw)
 
 
 def same(a, b):
@@ -111,3 +97,22 @@ def test_invalid_arguments(TurboSched):
     assert e.value.code == tc.TS_ERR_INVALID
     r = g.ts_sched_event([])
     assert r["M"] == 1 and r["phi"] == {}
+
+
+def test_replay_ablations_behave_as_the_paper_describes(TurboSched):
+    """paper_2606_19271_b200.sched_sim on 600 synthetic events: the closed loop never leaves an active session without a GPU
+    and never exceeds l_hat(K); a fixed budget of the same mean size does leave sessions unplaced in bursts; provisioning for
+    the peak costs far more GPU-events (§3.2 A2, §7.3); rebalancing only ever lowers the bottleneck (Eq. 4)."""
+    from paper_2606_19271_b200 import sched_sim
+    l_hat = sched_sim.LHAT_WAN13B_MS
+    ev = lambda: synth.sched_events(3, 600, cap=5 * 12)
+    full = sched_sim.replay(ev(), 5, 12, 1, l_hat, 0.7, 0.1, eta=0.05)
+    nomig = sched_sim.replay(ev(), 5, 12, 1, l_hat, 0.7, 0.1, eta=1e9)
+    fixed = max(1, round(full["mean_gpus"]))
+    same_budget = sched_sim.replay(ev(), 5, fixed, fixed, l_hat, 0.7, 10.0, eta=0.05)
+    peak = sched_sim.replay(ev(), 5, 12, 12, l_hat, 0.7, 10.0, eta=0.05)
+    assert full["unplaced_session_events"] == 0 and full["worst_case_latency_ms"] <= l_hat[5]
+    assert same_budget["unplaced_session_events"] > 0
+    assert peak["gpu_events"] > 1.5 * full["gpu_events"] and peak["unplaced_session_events"] == 0
+    assert full["mean_bottleneck_latency_ms"] <= nomig["mean_bottleneck_latency_ms"] + 1e-9
+    assert full["migrations"] > nomig["migrations"]
