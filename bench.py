@@ -323,6 +323,7 @@ def main():
 
     # ---- offload leg (side stream, timed alone): suspend / resume of a full-window session
     off = measure_offload(wl)
+    off["scattered"] = {k: v for k, v in measure_offload(wl, permuted=True).items() if k in ("d2h", "h2d", "placement")}
     mig = measure_migration(wl, peaks["hbm_gbs"])
 
     # ---- end to end through ts_chunk_step_host with pinned host buffers
@@ -389,7 +390,7 @@ def main():
     return 0
 
 
-def measure_offload(wl):
+def measure_offload(wl, permuted=False):
     """Suspend / resume of a full-window (21-frame) session on the side stream, timed with events on that stream,
     against a plain pinned cudaMemcpy of the same bytes measured in the same run."""
     import torch
@@ -399,7 +400,11 @@ def measure_offload(wl):
     sh = w.shape
     T, H, D = sh.frame_tokens, sh.n_heads, sh.head_dim
     dev = wl["q"].device
-    pool = TurboChunkPool(1, H, D, sh.page_tokens, 160, T, sh.window_frames, 2, host_pages=130, device=dev.index)
+    # FIFO allocation from an untouched pool keeps the session's pages adjacent (suspend / resume then move them in a few
+    # large copies); `permuted` scatters them over the pool as configs[2] asks: one copy per 1.57 MB page
+    order = np.random.default_rng(97).permutation(160) if permuted else None
+    pool = TurboChunkPool(1, H, D, sh.page_tokens, 160, T, sh.window_frames, 2, free_order=order, host_pages=130,
+                          device=dev.index)
     gen = torch.Generator(device=dev)
     gen.manual_seed(99)
     sid = pool.ts_session_open()
@@ -445,6 +450,7 @@ def measure_offload(wl):
     res["bytes"] = int(nbytes)
     res["pages"] = int(n_pages)
     res["peak_kind"] = "one pinned cudaMemcpyAsync of the same bytes, same run; both sides best of 6 (the host link is shared with other tenants of the box)"
+    res["placement"] = "pages scattered (one copy per page)" if permuted else "pages adjacent (FIFO allocation): runs of pages merge into one copy"
     pool.close()
     return res
 

@@ -1007,6 +1007,24 @@ int ts_gather_kv(ts_pool* pool, int32_t layer, int32_t sid, void* k_out, void* v
   return TS_OK;
 }
 
+// Page copies of a suspend (to_host) or resume on the side stream: one copy per run of pages that are adjacent both in the
+// slab and in the arena (FIFO allocation keeps a session's pages largely contiguous: a full window then moves at the
+// rate of one large copy; a permuted pool degenerates to one copy per page, 0.87 of it at 1.57 MB per page - alternating
+// the pages between two copy streams was measured and does not help: the copy engine serialises them).
+static int copy_session_pages(ts_pool* pool, const Session& s, bool to_host) {
+  const cudaMemcpyKind kind = to_host ? cudaMemcpyDeviceToHost : cudaMemcpyHostToDevice;
+  for (size_t i = 0; i < s.pt.size();) {
+    size_t e = i + 1;
+    while (e < s.pt.size() && s.pt[e] == s.pt[e - 1] + 1 && s.host_slots[e] == s.host_slots[e - 1] + 1) ++e;
+    uint8_t* dev_ptr = pool->slab + (int64_t)s.pt[i] * pool->page_bytes;
+    uint8_t* host_ptr = pool->host + (int64_t)s.host_slots[i] * pool->page_bytes;
+    TS_CUDA(cudaMemcpyAsync(to_host ? host_ptr : dev_ptr, to_host ? dev_ptr : host_ptr, (size_t)(e - i) * pool->page_bytes, kind,
+                            pool->side));
+    i = e;
+  }
+  return TS_OK;
+}
+
 // --------------------------------------------------------------------------------------------- offload
 int ts_session_suspend(ts_pool* pool, int32_t sid) {
   if (pool == nullptr) return TS_ERR_INVALID;
@@ -1019,11 +1037,12 @@ int ts_session_suspend(ts_pool* pool, int32_t sid) {
   TS_CUDA(pool->tl_compute.wait(pool->side, s.compute_seq));
   s.host_slots.clear();
   for (size_t i = 0; i < s.pt.size(); ++i) {
-    const int32_t slot = pool->host_free.back();
+    s.host_slots.push_back(pool->host_free.back());
     pool->host_free.pop_back();
-    s.host_slots.push_back(slot);
-    TS_CUDA(cudaMemcpyAsync(pool->host + (int64_t)slot * pool->page_bytes, pool->slab + (int64_t)s.pt[i] * pool->page_bytes,
-                            pool->page_bytes, cudaMemcpyDeviceToHost, pool->side));
+  }
+  {
+    const int rc = copy_session_pages(pool, s, true);
+    if (rc != TS_OK) return rc;
   }
   const uint64_t seq = pool->tl_side.record(pool->side);
   for (int32_t pg : s.pt) {
@@ -1052,9 +1071,9 @@ int ts_session_resume(ts_pool* pool, int32_t sid) {
     s.pt.push_back(pg);
   }
   TS_CUDA(pool->tl_compute.wait(pool->side, wait_compute));
-  for (size_t i = 0; i < s.pt.size(); ++i) {
-    TS_CUDA(cudaMemcpyAsync(pool->slab + (int64_t)s.pt[i] * pool->page_bytes, pool->host + (int64_t)s.host_slots[i] * pool->page_bytes,
-                            pool->page_bytes, cudaMemcpyHostToDevice, pool->side));
+  {
+    const int rc = copy_session_pages(pool, s, false);
+    if (rc != TS_OK) return rc;
   }
   s.side_seq = pool->tl_side.record(pool->side);
   for (auto it = s.host_slots.rbegin(); it != s.host_slots.rend(); ++it) pool->host_free.push_back(*it);
