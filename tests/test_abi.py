@@ -80,3 +80,18 @@ def test_product_path_does_not_import_oracle():
             if f.endswith(".py"):
                 assert "paper_2606_19271_b200" not in open(os.path.join(dirpath, f)).read().replace(
                     "`paper_2606_19271_b200/`", ""), f
+
+
+def test_headers_are_plain_c(tmp_path):
+    """The boundary is a C ABI: both headers compile as C99 on their own (no C++ types, no torch types)."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("gcc not available")
+    src = tmp_path / "hdr.c"
+    src.write_text('#include "turbochunk.h"\n#include "turbochunk_sched.h"\n'
+                   "int main(void) { ts_pool_config c; ts_sched_config s; (void)c; (void)s; return 0; }\n")
+    res = subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-fsyntax-only",
+                          "-I", os.path.join(ROOT, "include"), str(src)], capture_output=True, text=True)
+    assert res.returncode == 0, res.stderr
