@@ -304,8 +304,22 @@ def test_config2_full_size_sampled_rows():
     err, ref = np.concatenate(errs), np.concatenate(refs)
     assert np.abs(err).max() <= 2e-2
     assert np.linalg.norm(err) / np.linalg.norm(ref) <= 5e-3
-    # property that holds at any size: appended bytes read back bit-exact for a sampled session
-    dp.append(0, sids, cf, dev_to_bits(dk), dev_to_bits(dv), dev=(dk, dv))
+    # the launch configuration bench.py times: ts_chunk_step, attention + append in ONE launch.  flags = 0 (as in the timed
+    # loop) leaves the state alone and must reproduce the attention-only output bit for bit (every work item is computed
+    # the same way whichever cluster takes it); with TS_COMMIT the appended bytes read back bit-exact (a property that
+    # holds at any size) and the page tables match the oracle's.
+    import paper_2606_19271_b200 as tc
+    out2 = torch.full_like(dq, float("nan"))
+    lse2 = torch.empty_like(lse)
+    dp.g.ts_chunk_step(0, sids, cf, dq, dk, dv, out2, lse2, float(w.scale), 0)
+    torch.cuda.synchronize()
+    assert torch.equal(out.view(torch.int16), out2.view(torch.int16)) and torch.equal(lse, lse2)
+    out3 = torch.full_like(dq, float("nan"))
+    dp.o.append(0, sids, cf, dev_to_bits(dk), dev_to_bits(dv))
+    dp.g.ts_chunk_step(0, sids, cf, dq, dk, dv, out3, None, float(w.scale), tc.TS_COMMIT)
+    torch.cuda.synchronize()
+    assert torch.equal(out.view(torch.int16), out3.view(torch.int16))
+    dp.check_state(sids, kv=False)
     dp.check_state(sids[:2], kv=True)
 
 
