@@ -146,7 +146,7 @@ class OraclePool:
         for sid, c in zip(sids, chunk_frames):
             s = self.sessions[sid]
             end = s.o + s.P * T + c * T
-            need.append(-(-end // B) - len(s.PT))
+            need.append(max(0, -(-end // B) - len(s.PT)))       # R14: growth is idempotent, a table never shrinks on append
         if sum(need) > len(self.free):
             raise OracleError(NO_PAGES, "append needs more pages than are free")   # all-or-nothing
         off = 0

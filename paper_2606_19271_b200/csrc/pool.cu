@@ -211,12 +211,21 @@ static int check_batch(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
     total += (int64_t)cf[b] * c.frame_tokens;
   }
   if (total > (int64_t)1 << 30) return TS_ERR_INVALID;
+  // a malformed batch (the same id twice, R13) is TS_ERR_INVALID whatever the state of its sessions; states come second
+  for (int b = 0; b < n; ++b) {
+    const int sid = sids[b];
+    if (sid < 0 || sid >= c.max_sessions) {
+      for (int a = 0; a < b; ++a)
+        if (sids[a] == sid) return TS_ERR_INVALID;
+      continue;
+    }
+    if (mark[sid]) return TS_ERR_INVALID;
+    mark[sid] = 1;
+  }
   for (int b = 0; b < n; ++b) {
     const int sid = sids[b];
     if (sid < 0 || sid >= c.max_sessions) return TS_ERR_STATE;
     if (pool->sess[sid].state == TS_SESSION_CLOSED) return TS_ERR_STATE;
-    if (mark[sid]) return TS_ERR_INVALID;
-    mark[sid] = 1;
   }
   for (int b = 0; b < n; ++b)
     if (pool->sess[sids[b]].state != TS_SESSION_RESIDENT) return TS_ERR_STATE;

@@ -418,3 +418,25 @@ def test_state_machine_errors():
         pool.close(a)
     assert e.value.kind == oracle.STATE
     assert pool.open() == a                                                        # lowest free id reused
+
+
+def test_page_demand_is_never_negative():
+    """R14: page growth on append is idempotent and a table never shrinks, so a session that already holds more pages than
+    a later, smaller append needs contributes ZERO demand - it must not offset another session's demand in the all-or-nothing
+    check (found by the random-operation test: the unclamped sum let an append through that then ran out of pages)."""
+    shape = small_shape(n_pages=6, max_sessions=2)            # B = 8, T = 5
+    T = shape.frame_tokens
+    rng = np.random.default_rng(23)
+    pool = make_oracle_pool(shape)
+    a, b = pool.open(), pool.open()
+    pool.append(0, [a], [6], draw(rng, 6 * T, shape), draw(rng, 6 * T, shape), commit=False)   # 30 tokens: 4 pages, P stays 0
+    assert len(pool.page_table(a)) == 4 and len(pool.free) == 2
+    snap = (list(pool.free), pool.page_table(a), pool.page_table(b))
+    # a needs ceil(5 / 8) = 1 page and holds 4 (demand 0, not -3); b needs ceil(20 / 8) = 3 > 2 free
+    k = draw(rng, 5 * T, shape)
+    with pytest.raises(oracle.OracleError) as e:
+        pool.append(0, [a, b], [1, 4], k, k)
+    assert e.value.kind == oracle.NO_PAGES
+    assert snap == (list(pool.free), pool.page_table(a), pool.page_table(b))
+    pool.append(0, [a, b], [1, 3], k[:4 * T], k[:4 * T])      # b: 15 tokens = 2 pages: fits exactly
+    assert len(pool.free) == 0 and len(pool.page_table(a)) == 4 and len(pool.page_table(b)) == 2
