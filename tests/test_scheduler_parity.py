@@ -116,3 +116,24 @@ def test_replay_ablations_behave_as_the_paper_describes(TurboSched):
     assert peak["gpu_events"] > 1.5 * full["gpu_events"] and peak["unplaced_session_events"] == 0
     assert full["mean_bottleneck_latency_ms"] <= nomig["mean_bottleneck_latency_ms"] + 1e-9
     assert full["migrations"] > nomig["migrations"]
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_configurations_parity(TurboSched, seed):
+    """Random controller parameters (caps, budgets, latency tables with plateaus, hysteresis, eta / kappa, volatility tables)
+    on 120-event streams: the library and the oracle agree on every event (200 such seeds were run once without a mismatch)."""
+    rng = np.random.default_rng(seed)
+    K = int(rng.integers(1, 9))
+    M_max = int(rng.integers(1, 14))
+    l_hat = [0.0] + [float(x) for x in np.cumsum(rng.choice([0.0, 1.0, 50.0, 83.5], size=K))]
+    cfg = dict(K=K, M_max=M_max, M0=int(rng.integers(1, M_max + 1)), l_hat=l_hat,
+               rho_hat=float(rng.choice([0.3, 0.5, 0.7, 0.9, 1.0])), delta=float(rng.choice([0.0, 0.05, 0.1, 0.3])),
+               eta=float(rng.choice([0.0, 0.01, 0.37, 5.0])), kappa_alpha=float(rng.choice([0.0, 23.0])),
+               kappa_beta=float(rng.choice([0.0, 0.0371, 0.5])))
+    if rng.random() < 0.4:
+        levels = int(rng.integers(1, 6))
+        cfg.update(vol_window=int(rng.integers(1, 12)), vol_bounds=sorted(float(x) for x in rng.random(levels - 1) * 3),
+                   vol_rho=[float(x) for x in rng.choice([0.4, 0.6, 0.8, 0.95], size=levels)])
+    o, g = SchedulerOracle(**cfg), TurboSched(**cfg)
+    for ev in synth.sched_events(seed, 120, cap=K * M_max + 5, mean_on=float(rng.choice([1.0, 3.0, 8.0]))):
+        same(o.event(ev), g.ts_sched_event(ev))
