@@ -137,7 +137,9 @@ class TurboChunkPool:
     """Owns a ts_pool and the torch memory behind it.  Methods mirror the C ABI one to one."""
 
     def __init__(self, n_layers, n_heads, head_dim, page_tokens, n_pages, frame_tokens, window_frames,
-                 max_sessions, free_order=None, host_pages=0, device=0):
+                 max_sessions, free_order=None, host_pages=0, device=0, guard_bytes=0):
+        """guard_bytes > 0 (tests): the KV slab and the pinned arena sit between two guard bands of that many bytes filled
+        with 0xA5; `check_guards()` tells whether any library write strayed outside them."""
         cfg = ts_pool_config()
         cfg.n_layers, cfg.n_heads, cfg.head_dim, cfg.page_tokens = n_layers, n_heads, head_dim, page_tokens
         cfg.n_pages, cfg.frame_tokens, cfg.window_frames, cfg.max_sessions = n_pages, frame_tokens, window_frames, max_sessions
@@ -149,15 +151,25 @@ class TurboChunkPool:
         slab_bytes = int(lib.ts_pool_slab_bytes(C.byref(cfg)))
         self.device = torch.device("cuda", device)
         # device memory and pinned memory come from torch (PyTorch is the allocator, not the product)
-        self._slab = torch.empty(slab_bytes + 1024, dtype=torch.uint8, device=self.device)
+        guard = (int(guard_bytes) + 1023) // 1024 * 1024
+        self._guard = guard
+        self._slab = torch.empty(slab_bytes + 1024 + 2 * guard, dtype=torch.uint8, device=self.device)
         base = self._slab.data_ptr()
-        aligned = (base + 1023) // 1024 * 1024
+        aligned = (base + guard + 1023) // 1024 * 1024
+        self._slab_off = aligned - base
         cfg.kv_slab = aligned
         cfg.kv_slab_bytes = slab_bytes
+        self._slab_bytes = slab_bytes
+        if guard:
+            self._slab[:self._slab_off].fill_(0xA5)
+            self._slab[self._slab_off + slab_bytes:].fill_(0xA5)
         self._host = None
         if host_pages > 0:
-            self._host = torch.empty(host_pages * self.page_bytes, dtype=torch.uint8, pin_memory=True)
-            cfg.host_arena = self._host.data_ptr()
+            self._host = torch.empty(host_pages * self.page_bytes + 2 * guard, dtype=torch.uint8, pin_memory=True)
+            if guard:
+                self._host[:guard].fill_(0xA5)
+                self._host[guard + host_pages * self.page_bytes:].fill_(0xA5)
+            cfg.host_arena = self._host.data_ptr() + guard
             cfg.host_bytes = host_pages * self.page_bytes
         self._free_order = None
         if free_order is not None:
@@ -170,6 +182,18 @@ class TurboChunkPool:
         handle = C.c_void_p()
         _check(lib.ts_pool_create(C.byref(cfg), C.byref(handle)), "ts_pool_create")
         self._h = handle
+
+    def check_guards(self):
+        """True if the guard bands around the KV slab and the pinned arena still hold their fill pattern."""
+        if not self._guard:
+            return True
+        torch.cuda.synchronize(self.device)
+        ok = bool((self._slab[:self._slab_off] == 0xA5).all()) and \
+            bool((self._slab[self._slab_off + self._slab_bytes:] == 0xA5).all())
+        if self._host is not None:
+            n = self._host.numel()
+            ok = ok and bool((self._host[:self._guard] == 0xA5).all()) and bool((self._host[n - self._guard:] == 0xA5).all())
+        return ok
 
     # ---- lifecycle
     def close(self):

@@ -70,7 +70,7 @@ class DualPool:
         self.o = make_oracle_pool(shape, free_order, host_pages if host_pages else None)
         self.g = TurboChunkPool(shape.n_layers, shape.n_heads, shape.head_dim, shape.page_tokens, shape.n_pages,
                                 shape.frame_tokens, shape.window_frames, shape.max_sessions,
-                                free_order=free_order, host_pages=host_pages)
+                                free_order=free_order, host_pages=host_pages, guard_bytes=1 << 20)
 
     def open(self):
         a, b = self.o.open(), self.g.ts_session_open()
@@ -128,6 +128,8 @@ class DualPool:
 
     def check_state(self, sids, layers=None, kv=True):
         import torch
+        # compute-sanitizer is closed on the GPU pool: 1 MiB guard bands around the slab and the pinned arena stand in for it
+        assert self.g.check_guards(), "a library write strayed outside the KV slab or the pinned arena"
         assert list(self.o.free) == self.g.ts_pool_free_list()
         st_o, st_g = self.o.stats(), self.g.ts_pool_stats()
         for key in ("free_pages", "resident", "suspended", "host_pages_used"):
