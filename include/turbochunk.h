@@ -147,6 +147,10 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
  * `layer` (byte-exact 128-bit copies).  With TS_COMMIT: P += c, then roll the window: evict e = max(0, P - W)
  * oldest whole frames, o += e*T, pages whose slots are all dead go to the back of the free list (R6, R10).
  *   k, v : device bf16 [sum_b C_b][H][D] as above.
+ * Multi-layer protocol (R14): one step appends the SAME batch and chunk_frames to every layer and passes TS_COMMIT on the
+ * last one; a table never shrinks on append (a session that already holds more pages than a call needs contributes no
+ * demand), and the slots of the last page behind the appended tokens are zero-filled, so an uncommitted append must not be
+ * followed by a shorter one to the same layer before the commit.
  */
 int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*host*/,
                  const int32_t* chunk_frames /*host*/, const void* k, const void* v, uint32_t flags,
