@@ -17,7 +17,11 @@ visible key, P4 placement invariance, P5 suspend/resume identity, P6 reduction t
 torch SDPA, P7 chunked == monolithic, P8 batch-composition invariance, P9 softmax
 invariants + LSE merge, P10 window equivalence + page-count closed forms, P11
 hand-worked allocator trace (tests/golden/tiny_allocator_trace.txt), P12 distribution
-sanity; migration (O4, `OraclePool.migrate_to`): M1 hand-worked id trace
+sanity, P13 `attention_rows` (the sampled-row entry point of the full-size parity tests and
+of bench.py's cpu_baseline) against `chunk_attention` on a rolled-window multi-head pool
+and against explicit loops over the logical arrays, P14 the bf16 conversions (`_widen`,
+synth.bf16) against torch.bfloat16 on all 65 536 patterns / 1.4 M fp32 values incl. ties;
+migration (O4, `OraclePool.migrate_to`): M1 hand-worked id trace
 (tests/golden/migration_trace.txt), M2 == suspend + transplant + resume, M3 round trip and
 attention invariance, M4 conservation.  Parity unpinned: none.
 """

@@ -440,3 +440,131 @@ def test_page_demand_is_never_negative():
     assert snap == (list(pool.free), pool.page_table(a), pool.page_table(b))
     pool.append(0, [a, b], [1, 3], k[:4 * T], k[:4 * T])      # b: 15 tokens = 2 pages: fits exactly
     assert len(pool.free) == 0 and len(pool.page_table(a)) == 4 and len(pool.page_table(b)) == 2
+
+
+# ---- P13: attention_rows — the function behind every sampled-row parity check and the timed CPU baseline ----
+def _rolled_multihead_pool():
+    """W binding (P + c > W), o != 0, permuted pages, 3 heads, a second session sharing the pool."""
+    shape = small_shape(n_heads=3, head_dim=16, window_frames=6, page_tokens=8, frame_tokens=5, n_pages=48)
+    T = shape.frame_tokens
+    rng = np.random.default_rng(31)
+    pool = make_oracle_pool(shape, rng.permutation(shape.n_pages))
+    other, sid = pool.open(), pool.open()
+    prior_k, prior_v = draw(rng, 11 * T, shape), draw(rng, 11 * T, shape)
+    fed = 0
+    for c in (3, 2, 3, 3):                                   # 11 frames through a 6-frame window: 5 evicted, o = 25 % 8 = 1
+        sl = slice(fed * T, (fed + c) * T)
+        pool.append(0, [sid], [c], prior_k[sl], prior_v[sl])
+        pool.append(0, [other], [1], draw(rng, T, shape), draw(rng, T, shape))   # interleaves the page ids
+        fed += c
+    info = pool.info(sid)
+    assert info["frames"] == 6 and info["head_off"] == 1
+    return shape, pool, sid, other, prior_k, prior_v, rng
+
+
+def _same_up_to_blas_order(a, b):
+    # the two entry points hand numpy's fp64 matmul different row counts (gemv / gemm blocking differs), so the sums
+    # are taken in a different order: a few ulp, nothing a wrong index or mask could hide behind
+    np.testing.assert_allclose(a, b, rtol=1e-12, atol=1e-14)
+
+
+def test_p13_attention_rows_equals_chunk_attention():
+    # (a) rolled-window multi-head pool: arbitrary unsorted, repeated row subsets, every head, O and LSE
+    shape, pool, sid, other, _, _, rng = _rolled_multihead_pool()
+    T, H = shape.frame_tokens, shape.n_heads
+    c = 3
+    q, k, v = (draw(rng, c * T, shape) for _ in range(3))
+    qo, ko, vo = (draw(rng, 2 * T, shape) for _ in range(3))
+    # the session sits SECOND in a two-session batch, so the packed offset of its chunk is not 0
+    qa, ka, va = (np.concatenate([x, y]) for x, y in ((qo, q), (ko, k), (vo, v)))
+    O, LSE = oracle.chunk_attention(pool, 0, [other, sid], [2, c], qa, ka, va, np.float32(0.21))
+    off = 2 * T
+    for rows in ([0], [c * T - 1], [7, 2, 11, 2, 14, 0, 5], list(range(c * T))[::-1], rng.permutation(c * T)[:6].tolist()):
+        for h in range(H):
+            o, l = oracle.attention_rows(pool, 0, sid, c, q, k, v, np.float32(0.21), h, rows)
+            _same_up_to_blas_order(o, O[off + np.asarray(rows), h])
+            _same_up_to_blas_order(l, LSE[off + np.asarray(rows), h])
+    # ... and on Tiny (no window, D = 64, B = T = 16)
+    w = synth.tiny()
+    tpool, sids, tensors, tq, tk, tv = build_oracle_workload(w)
+    cf = [s.chunk_frames for s in w.sessions]
+    TO, TL = oracle.chunk_attention(tpool, 0, sids, cf, tq, tk, tv, w.scale)
+    off = 0
+    for s, spec, t in zip(sids, w.sessions, tensors):
+        Cn = spec.chunk_frames * w.shape.frame_tokens
+        rows = [Cn - 1, 0, 17, 3, 16, 15]
+        for h in range(w.shape.n_heads):
+            o, l = oracle.attention_rows(tpool, 0, s, spec.chunk_frames, t["q"], t["k"], t["v"], w.scale, h, rows)
+            _same_up_to_blas_order(o, TO[off + np.asarray(rows), h])
+            _same_up_to_blas_order(l, TL[off + np.asarray(rows), h])
+        off += Cn
+
+
+def test_p13_attention_rows_brute_force():
+    # (b) hand-picked rows against explicit loops over the LOGICAL arrays (as drawn: no page table, no oracle helper):
+    # a row of the first frame, one of the middle frame (last token of it) and the very last row, a different head each.
+    shape, pool, sid, _, prior_k, prior_v, rng = _rolled_multihead_pool()
+    T, D, Wn = shape.frame_tokens, shape.head_dim, shape.window_frames
+    c = 3
+    q, k, v = (draw(rng, c * T, shape) for _ in range(3))
+    scale = np.float32(0.37)
+    n_fed = prior_k.shape[0] // T                      # 11 frames were fed; the cache holds the last 6; W - c = 3 are visible
+    vis_lo = (n_fed - (Wn - c)) * T
+    Kp, Vp = W64(prior_k)[vis_lo:], W64(prior_v)[vis_lo:]
+    Q, Kc, Vc = W64(q), W64(k), W64(v)
+    assert Kp.shape[0] == (Wn - c) * T
+    for row, head in ((2, 0), (2 * T - 1, 1), (c * T - 1, 2)):
+        den, num = 0.0, [0.0] * D
+        keys = [(Kp[j, head], Vp[j, head]) for j in range(Kp.shape[0])]
+        keys += [(Kc[j, head], Vc[j, head]) for j in range(c * T) if j // T <= row // T]
+        for kk, vv in keys:
+            dot = 0.0
+            for d in range(D):
+                dot += Q[row, head, d] * kk[d]
+            e = math.exp(float(scale) * dot)
+            den += e
+            for d in range(D):
+                num[d] += e * vv[d]
+        o, l = oracle.attention_rows(pool, 0, sid, c, q, k, v, scale, head, [row])
+        np.testing.assert_allclose(o[0], np.array(num) / den, rtol=1e-11, atol=1e-13)
+        assert abs(l[0] - math.log(den)) < 1e-11
+    # a transposed head axis or rows-as-positions slip would show here: the three rows differ from each other's heads
+    o_wrong, _ = oracle.attention_rows(pool, 0, sid, c, q, k, v, scale, 1, [2])
+    o_right, _ = oracle.attention_rows(pool, 0, sid, c, q, k, v, scale, 0, [2])
+    assert np.abs(o_wrong - o_right).max() > 1e-3
+
+
+# ---- P14: the bf16 conversions against a library (torch.bfloat16 on CPU) ----------------------------------
+def test_p14_bf16_widening_all_patterns_vs_torch():
+    from oracle.attention import _widen
+    bits = np.arange(65536, dtype=np.uint32).astype(np.uint16)
+    ref32 = torch.from_numpy(bits.view(np.int16)).view(torch.bfloat16).to(torch.float32).numpy()
+    ref64 = torch.from_numpy(bits.view(np.int16)).view(torch.bfloat16).to(torch.float64).numpy()
+    for got, ref in ((synth.bf16_bits_to_f32(bits), ref32), (synth.bf16_bits_to_f64(bits), ref64), (_widen(bits), ref64)):
+        assert got.dtype == ref.dtype
+        nan = np.isnan(ref)
+        assert np.array_equal(np.isnan(got), nan)
+        # bit-for-bit on every non-NaN pattern (incl. +-0, subnormals, +-inf)
+        view = np.uint32 if ref.dtype == np.float32 else np.uint64
+        assert np.array_equal(got[~nan].view(view), ref[~nan].view(view))
+    assert int(np.isnan(ref32).sum()) == 2 * 127                       # sanity: the NaN patterns were in the sweep
+
+
+def test_p14_f32_to_bf16_rne_vs_torch():
+    rng = np.random.default_rng(41)
+    x = rng.standard_normal(1_000_000, dtype=np.float32) * np.float32(3.0)
+    # exact ties (low 16 bits == 0x8000) with even and odd kept mantissas, values just below / above a tie, a mantissa carry
+    # into the exponent (0x3F7FFFFF -> 1.0), signed zeros, subnormals, the largest finite fp32 that stays finite in bf16
+    u = rng.integers(0, 0x7F000000, size=200_000, dtype=np.uint32)
+    ties = (u & np.uint32(0xFFFF0000)) | np.uint32(0x8000)
+    near = np.concatenate([ties - np.uint32(1), ties + np.uint32(1)])
+    special = np.array([0x3F7FFFFF, 0x3F7F8000, 0x3F808000, 0x3F818000, 0x00000000, 0x80000000, 0x00000001, 0x00008000,
+                        0x00018000, 0x7F7F0000, 0x7F7F7FFF, 0xBF7FFFFF], dtype=np.uint32)
+    allu = np.concatenate([x.view(np.uint32), ties, ties | np.uint32(0x80000000), near, special])
+    xs = allu.view(np.float32)
+    assert np.isfinite(xs).all()
+    ref = torch.from_numpy(xs.copy()).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+    got = synth.f32_to_bf16_bits(xs)
+    assert np.array_equal(got, ref)
+    # round trip: widening the rounded value and rounding again is the identity
+    assert np.array_equal(synth.f32_to_bf16_bits(synth.bf16_bits_to_f32(got)), got)
