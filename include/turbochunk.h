@@ -78,7 +78,11 @@ typedef struct ts_pool_config {
   const int32_t* free_order; /* host */
   /* KV slab: device memory of at least ts_pool_slab_bytes() bytes, 1024-byte aligned.  NULL: the library
    * allocates it with cudaMalloc.  Caller-provided memory (e.g. a torch tensor) stays owned by the caller
-   * and must outlive the pool. */
+   * and must outlive the pool.  The slab needs NO initialisation and is never cleared: no result depends on a
+   * byte the library has not written itself ("isolated per-session state regions").  The
+   * attention gathers only table entries that hold a cached token of the session; the slots of those pages
+   * that hold no visible token (dead head slots, the tail behind the last token) are masked, and they are
+   * the session's own older tokens or the append's zero fill. */
   void* kv_slab;          /* device */
   int64_t kv_slab_bytes;
   /* Pinned host arena for suspended sessions, in whole pages of ts_pool_page_bytes().  NULL with

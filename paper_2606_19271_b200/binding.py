@@ -137,9 +137,12 @@ class TurboChunkPool:
     """Owns a ts_pool and the torch memory behind it.  Methods mirror the C ABI one to one."""
 
     def __init__(self, n_layers, n_heads, head_dim, page_tokens, n_pages, frame_tokens, window_frames,
-                 max_sessions, free_order=None, host_pages=0, device=0, guard_bytes=0):
+                 max_sessions, free_order=None, host_pages=0, device=0, guard_bytes=0, poison=None):
         """guard_bytes > 0 (tests): the KV slab and the pinned arena sit between two guard bands of that many bytes filled
-        with 0xA5; `check_guards()` tells whether any library write strayed outside them."""
+        with 0xA5; `check_guards()` tells whether any library write strayed outside them.
+        poison (tests): a 16-bit pattern (0x7FC0 = bf16 NaN, 0x7F7F = the largest finite bf16) the whole slab is filled
+        with before ts_pool_create; `poison_free_pages()` refills the pages on the free list.  The library needs no
+        initialised slab (turbochunk.h): a result must never depend on bytes it has not written itself."""
         cfg = ts_pool_config()
         cfg.n_layers, cfg.n_heads, cfg.head_dim, cfg.page_tokens = n_layers, n_heads, head_dim, page_tokens
         cfg.n_pages, cfg.frame_tokens, cfg.window_frames, cfg.max_sessions = n_pages, frame_tokens, window_frames, max_sessions
@@ -163,6 +166,9 @@ class TurboChunkPool:
         if guard:
             self._slab[:self._slab_off].fill_(0xA5)
             self._slab[self._slab_off + slab_bytes:].fill_(0xA5)
+        self._poison = poison
+        if poison is not None:
+            self._slab[self._slab_off:self._slab_off + slab_bytes].view(torch.int16).fill_(int(poison) - (1 << 16 if poison >= 1 << 15 else 0))
         self._host = None
         if host_pages > 0:
             self._host = torch.empty(host_pages * self.page_bytes + 2 * guard, dtype=torch.uint8, pin_memory=True)
@@ -194,6 +200,18 @@ class TurboChunkPool:
             n = self._host.numel()
             ok = ok and bool((self._host[:self._guard] == 0xA5).all()) and bool((self._host[n - self._guard:] == 0xA5).all())
         return ok
+
+    def poison_free_pages(self):
+        """(tests) Refill every page on the free list with the poison pattern.  Synchronises the device first: a page on
+        the free list may still be the source of a suspend's copy or the operand of an enqueued kernel."""
+        if self._poison is None:
+            return
+        torch.cuda.synchronize(self.device)
+        body = self._slab[self._slab_off:self._slab_off + self._slab_bytes].view(torch.int16).view(-1, self.page_bytes // 2)
+        ids = self.ts_pool_free_list()
+        if ids:
+            body[torch.tensor(ids, dtype=torch.long, device=self.device)] = int(self._poison) - (1 << 16 if self._poison >= 1 << 15 else 0)
+        torch.cuda.synchronize(self.device)
 
     # ---- lifecycle
     def close(self):

@@ -45,11 +45,11 @@ constexpr int kPolyPairs = 4;
 
 // 2^x for a pair on the FMA pipe (Cody-Waite): x = n + f with n = round(x), f in [-0.5, 0.5]; 2^f by a degree-3 minimax
 // polynomial (max relative error 7.5e-5, far below the 2^-9 of the bf16 rounding of P); 2^n as the fp32 whose bits are
-// (n + 127) << 23 - n + 127 sits in the low mantissa bits of x + (1.5 * 2^23 + 127).  x is clamped at -125 (masked
-// scores are -inf), which yields 2^-125 instead of 0: negligible against a row sum >= 1.
+// (n + 127) << 23 - n + 127 sits in the low mantissa bits of x + (1.5 * 2^23 + 127).  x is clamped at -127 (masked
+// scores are -inf): n + 127 = 0 there, the scale factor is +0.0 and p is exactly 0, as on the MUFU path.
 __device__ __forceinline__ void exp2_poly_pair(float x0, float x1, float& p0, float& p1) {
-  x0 = fmaxf(x0, -125.f);
-  x1 = fmaxf(x1, -125.f);
+  x0 = fmaxf(x0, -127.f);
+  x1 = fmaxf(x1, -127.f);
   float f0, f1, n0, n1, r0, r1, q0, q1;
   addc2(f0, f1, x0, x1, 12583039.f);
   addc2(n0, n1, f0, f1, -12583039.f);
@@ -233,7 +233,11 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
               if (j < g.n_prior) {
                 const CUtensorMap* mc = kv ? &p.map_v : &p.map_k;
                 const int x = ((g.t0 + j) << 7) + sx * sb;            // page-table coordinate of the box
-                const int page = pt[min(x >> p.log2_B, g.n_pt - 1)];  // past-the-end boxes re-read the last page (masked)
+                // Boxes past the last cached token re-read the last page that HOLDS a cached token (masked): its tail is
+                // real data or the append's zero fill.  Never a later table entry: a fused step and layers > 0 of a
+                // multi-layer step see tables already grown by pages whose bytes in this layer are not written yet
+                // (stale memory of a previous owner: P = 0 times a NaN there would be NaN inside the MMA).
+                const int page = pt[min(x >> p.log2_B, (g.x_end - 1) >> p.log2_B)];
                 const int tok = x & (p.B - 1);
                 for (int b = 0; b < C::kDBlocks; ++b) {
                   if (g.mc) tma_load_4d_mc(d + b * C::kBlockBytes, mc, 64 * b, tok, g.head, page, &kv_full[slot], 3);

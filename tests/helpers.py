@@ -63,14 +63,18 @@ class DualPool:
     (max-abs <= 2e-2, rel-L2 <= 5e-3 against fp64 — BASELINE.json north_star)."""
 
     MAX_ABS, REL_L2 = 2e-2, 5e-3
+    NAN_BF16, HUGE_BF16 = 0x7FC0, 0x7F7F
 
-    def __init__(self, shape, free_order=None, host_pages=0):
+    def __init__(self, shape, free_order=None, host_pages=0, poison=NAN_BF16):
+        """Every test pool starts with its whole KV slab filled with bf16 NaN (`poison`; None: torch.empty), and every state
+        check refills the pages on the free list: a result that depends on a byte the library has not written itself (a
+        stale page behind a grown table, a recycled page) turns into a NaN in the output instead of passing by luck."""
         from paper_2606_19271_b200 import TurboChunkPool
         self.shape = shape
         self.o = make_oracle_pool(shape, free_order, host_pages if host_pages else None)
         self.g = TurboChunkPool(shape.n_layers, shape.n_heads, shape.head_dim, shape.page_tokens, shape.n_pages,
                                 shape.frame_tokens, shape.window_frames, shape.max_sessions,
-                                free_order=free_order, host_pages=host_pages, guard_bytes=1 << 20)
+                                free_order=free_order, host_pages=host_pages, guard_bytes=1 << 20, poison=poison)
 
     def open(self):
         a, b = self.o.open(), self.g.ts_session_open()
@@ -126,6 +130,24 @@ class DualPool:
                 assert np.abs(l_gpu - lse_ref).max() <= 2e-3, float(np.abs(l_gpu - lse_ref).max())
         return o_gpu, o_ref
 
+    def fused_step(self, layer, sids, cf, q_bits, k_bits, v_bits, scale, commit=True, dev=None):
+        """ts_chunk_step (attention + append in one launch) against oracle attention followed by oracle append; the fused
+        launch's `out` is compared like a plain attention's."""
+        import torch
+        from paper_2606_19271_b200 import TS_COMMIT
+        o_ref, _ = oracle.chunk_attention(self.o, layer, sids, cf, q_bits, k_bits, v_bits, scale)
+        self.o.append(layer, sids, cf, k_bits, v_bits, commit=commit)
+        dq, dk, dv = dev if dev is not None else (bits_to_dev(q_bits), bits_to_dev(k_bits), bits_to_dev(v_bits))
+        out = torch.full_like(dq, float("nan"))
+        self.g.ts_chunk_step(layer, sids, cf, dq, dk, dv, out, None, float(scale), TS_COMMIT if commit else 0)
+        torch.cuda.synchronize()
+        o_gpu = out.double().cpu().numpy()
+        assert np.isfinite(o_gpu).all(), "fused step: non-finite output (a masked operand read bytes the library never wrote)"
+        max_abs = float(np.abs(o_gpu - o_ref).max())
+        rl2 = rel_l2(o_gpu, o_ref)
+        assert max_abs <= self.MAX_ABS and rl2 <= self.REL_L2, (max_abs, rl2)
+        return o_gpu, o_ref
+
     def check_state(self, sids, layers=None, kv=True):
         import torch
         # compute-sanitizer is closed on the GPU pool: 1 MiB guard bands around the slab and the pinned arena stand in for it
@@ -147,3 +169,4 @@ class DualPool:
                     ok, ov = self.o.gather_kv(layer, sid)
                     assert np.array_equal(dev_to_bits(gk), ok), f"K bytes differ sid={sid} layer={layer}"
                     assert np.array_equal(dev_to_bits(gv), ov), f"V bytes differ sid={sid} layer={layer}"
+        self.g.poison_free_pages()

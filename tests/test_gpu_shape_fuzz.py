@@ -1,7 +1,7 @@
 """Seeded shape fuzz of the coalesced step against the oracle: frame sizes from 1 token to several tiles, page sizes from 16
 to 512 tokens, 1-12 heads, both head dims, 1-8 sessions with ragged priors and chunk lengths, windows that clamp and roll,
-one or two layers, three softmax scales.  Each case runs attention (tolerance of the north_star), the fused step on every layer
-with the commit on the last (page tables, free list, KV bytes exact) and a second attention over the grown caches in reversed
+one or two layers, three softmax scales, on a NaN-poisoned slab.  Each case runs attention (tolerance of the north_star), the fused
+step on every layer with the commit on the last (its output against the oracle; page tables, free list, KV bytes exact) and a second attention over the grown caches in reversed
 batch order.  The work-tile scheduler sees pairs, odd items, lone tiles, single-tile plans and unrelated items sharing a
 cluster across these cases."""
 import numpy as np
@@ -43,11 +43,11 @@ def run_case(seed, large):
     scale = np.float32(rng.choice([0.05, 1.0 / np.sqrt(D), 0.3]))
     layer = int(rng.integers(0, NL))
     dp.attention(layer, sids, cf, q, k, v, scale)
-    dq, dk, dv = bits_to_dev(q), bits_to_dev(k), bits_to_dev(v)
-    out = torch.empty_like(dq)
+    dev = (bits_to_dev(q), bits_to_dev(k), bits_to_dev(v))
     for l in range(NL):
-        dp.o.append(l, sids, cf, k, v, commit=(l == NL - 1))
-        dp.g.ts_chunk_step(l, sids, cf, dq, dk, dv, out, None, float(scale), tc.TS_COMMIT if l == NL - 1 else 0)
+        # layer l > 0 runs on page tables that layer 0's uncommitted append has already grown: the slab is NaN-poisoned
+        # (DualPool), so a gather that strays onto a not-yet-written page shows up in `out`, which is compared here
+        dp.fused_step(l, sids, cf, q, k, v, scale, commit=(l == NL - 1), dev=dev)
     dp.check_state(sids)
     q2, k2, v2 = (synth.draw_bits(rng, n * T, H, D) for _ in range(3))
     dp.attention(layer, sids[::-1], [1] * n, q2, k2, v2, scale)
