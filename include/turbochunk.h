@@ -187,6 +187,54 @@ int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
                        const void* q_host, const void* k_host, const void* v_host, void* out_host,
                        float scale, uint32_t flags, void* cuda_stream);
 
+/*
+ * Capture-safe multi-layer chunk step.  PAPER.md:66 (iii): the worker "invokes the model once
+ * for the batch" - NL layers x several denoising passes of attention over the SAME batch and the same caches - "and
+ * writes the generated chunks and updated states back".  A plan splits ts_chunk_step into the part that depends on
+ * the sessions' state (once per chunk step, host + one upload) and the part that is repeated per layer and pass (one
+ * kernel launch and nothing else), so that the launches of a whole step can be captured into a CUDA graph once and
+ * replayed for every later chunk step of the same batch:
+ *
+ *   ts_step_plan_create(pool, n, sids, chunk_frames, n_slots, &plan)   batch composition and buffers are fixed per plan
+ *   ts_step_plan_bind(plan, slot, q, k, v, out, lse)                   n_slots sets of device tensors (e.g. one per layer,
+ *                                                                      or one reused by all layers)
+ *   per chunk step:
+ *     ts_step_plan_prepare(plan, stream)      NOT capturable.  Validates as ts_chunk_step (TS_ERR_STATE, TS_ERR_NO_PAGES;
+ *                                             all-or-nothing), grows the page tables for the step's append, builds the
+ *                                             schedule (a1) and writes it into the plan's device block in stream order
+ *                                             (one H2D of the whole block); enqueues the stream-side waits (pending
+ *                                             resumes, copies out of recycled pages).  The block's address, the grid
+ *                                             and every kernel argument are the same for every prepare of a plan.
+ *     ts_step_plan_run(plan, layer, slot, scale, run_flags, stream)
+ *                                             capturable: exactly one kernel launch, no copy, no event, no allocation.
+ *                                             Attention of `layer` on the tensors of `slot`; with TS_RUN_APPEND the
+ *                                             launch also appends the slot's K/V to `layer` (as ts_chunk_step does).
+ *                                             Any number of runs per step, in stream order (layers x passes).
+ *     ts_step_plan_commit(plan, flags, stream)  NOT capturable.  Ends the step: host bookkeeping of ts_kv_append(flags)
+ *                                             (TS_COMMIT: P += c and the window roll; 0: the tables stay grown, nothing
+ *                                             advances) and the event after which the step's launches count as done.
+ *   ts_step_plan_destroy(plan)
+ *
+ * Between prepare and commit the batch's sessions belong to the plan: every other call that names one of them
+ * (attention, append, step, suspend, close, migrate, another plan) returns TS_ERR_STATE.  Launches of one plan must not
+ * overlap in time (one stream, or ordered streams): they share the plan's work-item cursor, which each launch rearms
+ * for the next.  A graph captured between a prepare and a commit may be replayed after any later prepare of the same plan.
+ * Errors: create: as ts_chunk_attention's batch checks, TS_ERR_CUDA; bind: TS_ERR_INVALID (slot, null or misaligned
+ * pointer), TS_ERR_STATE (plan prepared); run: TS_ERR_STATE (not prepared, slot not bound), TS_ERR_INVALID.
+ */
+typedef struct ts_step_plan ts_step_plan; /* opaque */
+enum { TS_RUN_APPEND = 1u };              /* ts_step_plan_run flags */
+int ts_step_plan_create(ts_pool* pool, int32_t n, const int32_t* sids /*host*/, const int32_t* chunk_frames /*host*/,
+                        int32_t n_slots, ts_step_plan** out);
+int ts_step_plan_bind(ts_step_plan* plan, int32_t slot, const void* q, const void* k, const void* v, void* out,
+                      float* lse /*nullable*/); /* device bf16 [sum C][H][D] as ts_chunk_attention */
+int ts_step_plan_prepare(ts_step_plan* plan, void* cuda_stream);
+int ts_step_plan_run(ts_step_plan* plan, int32_t layer, int32_t slot, float scale, uint32_t run_flags, void* cuda_stream);
+int ts_step_plan_commit(ts_step_plan* plan, uint32_t flags, void* cuda_stream);
+int ts_step_plan_destroy(ts_step_plan* plan);
+/* Size of the plan's device block (tensor maps, descriptors, page tables, work items), for reporting. */
+int64_t ts_step_plan_block_bytes(ts_step_plan* plan);
+
 /* PAPER.md:76 (i)-(ii): copy the session's pages (every layer, whole pages, logical order — R11) to the pinned
  * arena on the side stream, after the compute-stream work already enqueued on that session; mark SUSPENDED;
  * push its page ids to the back of the free list in logical order.  A freed page is not handed to a later

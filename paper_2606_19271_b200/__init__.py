@@ -7,7 +7,7 @@ library is missing, and every compute call fails with TS_ERR_CUDA without an sm_
 """
 import importlib
 
-__all__ = ["TurboChunkError", "TurboChunkPool", "TurboSched", "lib", "lib_path", "TS_COMMIT", "TS_OK", "TS_ERR_INVALID",
+__all__ = ["TurboChunkError", "TurboChunkPool", "TurboSched", "StepPlan", "lib", "lib_path", "TS_COMMIT", "TS_RUN_APPEND", "TS_OK", "TS_ERR_INVALID",
            "TS_ERR_STATE", "TS_ERR_NO_PAGES", "TS_ERR_NO_HOST", "TS_ERR_CAPACITY", "TS_ERR_CUDA",
            "TS_SESSION_RESIDENT", "TS_SESSION_SUSPENDED", "EXPORTED_SYMBOLS"]
 

@@ -15,6 +15,7 @@ lib_path = os.path.join(HERE, "libturbochunk.so")
 TS_OK, TS_ERR_INVALID, TS_ERR_STATE, TS_ERR_NO_PAGES, TS_ERR_NO_HOST, TS_ERR_CAPACITY, TS_ERR_CUDA = 0, -1, -2, -3, -4, -5, -6
 TS_SESSION_CLOSED, TS_SESSION_RESIDENT, TS_SESSION_SUSPENDED = 0, 1, 2
 TS_COMMIT = 1
+TS_RUN_APPEND = 1
 
 EXPORTED_SYMBOLS = [
     "ts_pool_page_bytes", "ts_pool_slab_bytes", "ts_pool_create", "ts_pool_destroy", "ts_session_open",
@@ -22,6 +23,8 @@ EXPORTED_SYMBOLS = [
     "ts_session_resume", "ts_session_migrate", "ts_offload_sync", "ts_session_info", "ts_session_page_table", "ts_gather_kv",
     "ts_pool_free_list", "ts_pool_stats", "ts_pool_side_stream", "ts_pool_launch_count", "ts_strerror",
     "ts_last_cuda_error", "ts_version",
+    "ts_step_plan_create", "ts_step_plan_bind", "ts_step_plan_prepare", "ts_step_plan_run", "ts_step_plan_commit",
+    "ts_step_plan_destroy", "ts_step_plan_block_bytes",
     "ts_sched_create", "ts_sched_destroy", "ts_sched_event", "ts_sched_moves", "ts_sched_alive",
 ]
 
@@ -90,6 +93,14 @@ def _load():
     L.ts_pool_side_stream.argtypes = [P]
     L.ts_pool_launch_count.restype = C.c_int64
     L.ts_pool_launch_count.argtypes = [P]
+    L.ts_step_plan_create.argtypes = [P, C.c_int32, I32P, I32P, C.c_int32, C.POINTER(P)]
+    L.ts_step_plan_bind.argtypes = [P, C.c_int32, P, P, P, P, P]
+    L.ts_step_plan_prepare.argtypes = [P, P]
+    L.ts_step_plan_run.argtypes = [P, C.c_int32, C.c_int32, C.c_float, C.c_uint32, P]
+    L.ts_step_plan_commit.argtypes = [P, C.c_uint32, P]
+    L.ts_step_plan_destroy.argtypes = [P]
+    L.ts_step_plan_block_bytes.restype = C.c_int64
+    L.ts_step_plan_block_bytes.argtypes = [P]
     DP = C.POINTER(C.c_double)
     L.ts_sched_create.argtypes = [C.POINTER(ts_sched_config), C.POINTER(P)]
     L.ts_sched_destroy.argtypes = [P]
@@ -254,6 +265,10 @@ class TurboChunkPool:
                                       _ptr(k_host), _ptr(v_host), _ptr(out_host), C.c_float(float(scale)),
                                       C.c_uint32(flags), _stream(stream)), "ts_chunk_step_host")
 
+    def ts_step_plan_create(self, sids, chunk_frames, n_slots=1):
+        """A capture-safe multi-layer step plan for this batch (include/turbochunk.h); returns a StepPlan."""
+        return StepPlan(self, sids, chunk_frames, n_slots)
+
     def ts_session_suspend(self, sid):
         _check(lib.ts_session_suspend(self._h, sid), "ts_session_suspend")
 
@@ -309,6 +324,45 @@ class TurboChunkPool:
     @property
     def side_stream(self):
         return self._side
+
+
+class StepPlan:
+    """ctypes view of the ts_step_plan_* calls; keeps the bound tensors alive.  Marshalling only."""
+
+    def __init__(self, pool, sids, chunk_frames, n_slots=1):
+        h = C.c_void_p()
+        _check(lib.ts_step_plan_create(pool._h, len(sids), _i32(sids), _i32(chunk_frames), n_slots, C.byref(h)),
+               "ts_step_plan_create")
+        self._h, self._pool, self._keep = h, pool, {}
+
+    def ts_step_plan_bind(self, slot, q, k, v, out, lse=None):
+        _check(lib.ts_step_plan_bind(self._h, slot, _ptr(q), _ptr(k), _ptr(v), _ptr(out), _ptr(lse)), "ts_step_plan_bind")
+        self._keep[slot] = (q, k, v, out, lse)
+
+    def ts_step_plan_prepare(self, stream=None):
+        _check(lib.ts_step_plan_prepare(self._h, _stream(stream)), "ts_step_plan_prepare")
+
+    def ts_step_plan_run(self, layer, slot, scale, run_flags=TS_RUN_APPEND, stream=None):
+        _check(lib.ts_step_plan_run(self._h, layer, slot, C.c_float(float(scale)), C.c_uint32(run_flags), _stream(stream)),
+               "ts_step_plan_run")
+
+    def ts_step_plan_commit(self, flags=TS_COMMIT, stream=None):
+        _check(lib.ts_step_plan_commit(self._h, C.c_uint32(flags), _stream(stream)), "ts_step_plan_commit")
+
+    def ts_step_plan_block_bytes(self):
+        return int(lib.ts_step_plan_block_bytes(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib.ts_step_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            if getattr(self._pool, "_h", None):    # the pool must still exist: the plan points into it
+                self.close()
+        except Exception:
+            pass
 
 
 class TurboSched:

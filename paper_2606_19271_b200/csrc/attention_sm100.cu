@@ -21,6 +21,8 @@
 // CTA then loads half of every K/V tile and multicasts it to both (one L2 read per pair of CTAs); both CTAs cycle
 // the same number of tiles through their rings so that a tile sits at the same smem offset in both.  Every slot
 // release goes to the kv_empty barriers of both CTAs (count 2), also when the two CTAs work on unrelated items.
+#include <mutex>
+
 #include "internal.h"
 #include "kv_copy.cuh"
 #include "ptx.cuh"
@@ -86,13 +88,20 @@ struct ItemGeom {
 // takes the next one from a global cursor when it gets there (it runs ahead of every other role) and publishes it as
 // the k-th item of its cluster; every other role of both CTAs reads entry k of the cluster's ring.  An entry carries
 // its sequence number, so a stale value of the ring slot's previous use is never mistaken for it.  -1: no more items.
+// A fetcher sees the end of the list exactly once; the last cluster to see it sets the cursor back to zero (no fetcher
+// touches it again in this launch), and every cluster clears its own ring on exit: the block is rearmed for the next
+// launch by the kernel itself.
 __device__ __forceinline__ int next_cluster_item(const AttnParams& p, uint32_t k, bool fetcher) {
   unsigned long long* slot = p.feed + (size_t)(blockIdx.x >> 1) * kFeedRing + (k % kFeedRing);
   if (fetcher) {
-    int idx = atomicAdd(p.feed_counter, 1);
-    if (idx >= p.n_citems) idx = -1;
+    int idx = atomicAdd(p.feed_hdr, 1);
+    if (idx >= __ldg(p.feed_hdr + 2)) idx = -1;
     const unsigned long long v = ((unsigned long long)(k + 1) << 32) | (uint32_t)(idx + 1);
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(slot), "l"(v) : "memory");
+    if (idx < 0 && atomicAdd(p.feed_hdr + 1, 1) == (int)(gridDim.x >> 1) - 1) {
+      p.feed_hdr[1] = 0;
+      p.feed_hdr[0] = 0;
+    }
     return idx;
   }
   unsigned long long v;
@@ -621,21 +630,36 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
   __syncthreads();
   cluster_sync_all();   // no CTA exits while its partner may still multicast into it or arrive on its barriers
   if (warp == 1) tmem_dealloc(tmem_base, kTmemCols);
+  // every role of both CTAs has read the ring's last entry: clear it for the next launch on this block
+  if (cta_rank == 0 && threadIdx.x >= 64 && threadIdx.x < 64 + kFeedRing)
+    p.feed[(size_t)(blockIdx.x >> 1) * kFeedRing + (threadIdx.x - 64)] = 0ull;
 }
 
 int attention_smem_bytes(int head_dim) { return head_dim == 128 ? Cfg<128>::kSmemBytes : Cfg<64>::kSmemBytes; }
 
+// The dynamic shared memory limit is an attribute of the function on the CURRENT device: set once per device.
 template <int D>
-static cudaError_t launch_clustered(const AttnParams& p, int grid, cudaStream_t stream) {
-  static bool configured[64] = {};   // per device: the attribute belongs to the function on the CURRENT device
+static cudaError_t configure_once() {
+  static std::mutex mu;
+  static bool configured[64] = {};
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
   if (dev < 0 || dev >= 64 || !configured[dev]) {
     e = cudaFuncSetAttribute(chunk_attention_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<D>::kSmemBytes);
     if (e != cudaSuccess) return e;
     if (dev >= 0 && dev < 64) configured[dev] = true;
   }
+  return cudaSuccess;
+}
+
+cudaError_t attention_configure(int head_dim) { return head_dim == 128 ? configure_once<128>() : configure_once<64>(); }
+
+template <int D>
+static cudaError_t launch_clustered(const AttnParams& p, int grid, cudaStream_t stream) {
+  cudaError_t e = configure_once<D>();
+  if (e != cudaSuccess) return e;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid, 1, 1);
   cfg.blockDim = dim3(kThreads, 1, 1);

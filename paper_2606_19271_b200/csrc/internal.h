@@ -80,9 +80,11 @@ struct AttnParams {
   const SessDesc* sess;
   const int32_t* page_tables;
   const WorkItem* items;
-  unsigned long long* feed;      // [grid/2][kFeedRing] per-cluster ring of (sequence number, cluster item) pairs and
-  int32_t* feed_counter;         // the global cursor into the cluster-item list: see next_cluster_item()
-  int32_t n_citems;              // cluster items; items[2*i + r] is the work of CTA rank r for cluster item i
+  unsigned long long* feed;      // [grid/2][kFeedRing] per-cluster ring of (sequence number, cluster item) pairs
+  int32_t* feed_hdr;             // [0] the global cursor into the cluster-item list, [1] clusters that have seen its end,
+                                 // [2] n_citems (items[2*i + r] is the work of CTA rank r for cluster item i).  [0], [1] and
+                                 // the rings are zero at launch and zero again at exit (the kernel rearms them itself, so a
+                                 // captured launch can be replayed without a memset): see next_cluster_item()
   uint16_t* out;                 // bf16 [sum C][H][D]
   float* lse;                    // fp32 [sum C][H] or null
   int32_t H, T, B, log2_B;
@@ -98,5 +100,6 @@ cudaError_t launch_append(const CopyParams& p, int sm_count, cudaStream_t stream
 cudaError_t launch_gather(const CopyParams& p, int sm_count, cudaStream_t stream);
 cudaError_t launch_page_pull(const PullParams& p, int sm_count, cudaStream_t stream);
 int attention_smem_bytes(int head_dim);
+cudaError_t attention_configure(int head_dim);   // sets the kernel's dynamic shared memory limit on the current device (idempotent)
 
 }  // namespace tc

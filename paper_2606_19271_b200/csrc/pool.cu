@@ -47,41 +47,57 @@ static PFN_cuTensorMapEncodeTiled_v12000 get_encode() {
 // Every recorded event gets a monotonically increasing sequence number; objects (sessions, pages) remember the
 // sequence number after which they are safe to touch.
 struct EventTimeline {
-  static constexpr uint64_t kRing = 256;
-  cudaEvent_t ev[kRing];
-  uint64_t next_seq = 1;   // 0 means "nothing pending"
-  uint64_t done = 0;       // every seq <= done has completed
-  bool init() {
-    for (uint64_t i = 0; i < kRing; ++i)
-      if (cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming) != cudaSuccess) return false;
-    return true;
-  }
+  std::deque<cudaEvent_t> live;      // events of the sequence numbers done + 1 .. next_seq - 1, oldest first
+  std::vector<cudaEvent_t> spare;    // completed events, reused by record()
+  uint64_t next_seq = 1;             // 0 means "nothing pending"
+  uint64_t done = 0;                 // every seq <= done has completed
+  bool init() { return true; }
   void destroy() {
-    for (uint64_t i = 0; i < kRing; ++i) cudaEventDestroy(ev[i]);
+    for (cudaEvent_t e : live) cudaEventDestroy(e);
+    for (cudaEvent_t e : spare) cudaEventDestroy(e);
+    live.clear();
+    spare.clear();
   }
-  bool is_done(uint64_t seq) {
-    while (done < seq && done + 1 < next_seq) {
-      if (cudaEventQuery(ev[(done + 1) % kRing]) == cudaSuccess)
-        ++done;
-      else {
+  void retire() {                    // never waits: events that have completed go back to the spare list
+    while (!live.empty()) {
+      if (cudaEventQuery(live.front()) != cudaSuccess) {
         cudaGetLastError();
         break;
       }
+      spare.push_back(live.front());
+      live.pop_front();
+      ++done;
     }
+  }
+  bool is_done(uint64_t seq) {
+    if (done < seq) retire();
     return done >= seq;
   }
+  // The number of live events follows the work in flight (a few dozen); nothing here ever blocks the host.
   uint64_t record(cudaStream_t s) {
-    const uint64_t seq = next_seq++;
-    if (seq > kRing && done < seq - kRing) {   // the slot still belongs to an unfinished older event
-      cudaEventSynchronize(ev[seq % kRing]);
-      done = std::max(done, seq - kRing);
+    if (live.size() >= 64) retire();
+    cudaEvent_t e = nullptr;
+    if (!spare.empty()) {
+      e = spare.back();
+      spare.pop_back();
+    } else if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) {
+      cudaGetLastError();
+      // out of events: fall back to draining the stream once, then this sequence number is trivially complete
+      cudaStreamSynchronize(s);
+      retire();
+      return next_seq - 1;
     }
-    cudaEventRecord(ev[seq % kRing], s);
-    return seq;
+    cudaEventRecord(e, s);
+    live.push_back(e);
+    return next_seq++;
   }
   cudaError_t wait(cudaStream_t s, uint64_t seq) {
     if (seq == 0 || is_done(seq)) return cudaSuccess;
-    return cudaStreamWaitEvent(s, ev[seq % kRing], 0);
+    return cudaStreamWaitEvent(s, live[(size_t)(seq - done - 1)], 0);
+  }
+  void sync_all() {                  // pool teardown only
+    if (!live.empty()) cudaEventSynchronize(live.back());
+    retire();
   }
 };
 
@@ -94,6 +110,7 @@ struct Session {
   uint64_t compute_seq = 0;         // last compute-stream call that touched the session
   uint64_t side_seq = 0;            // last side-stream copy that touched the session
   uint64_t ver = 0;                 // new value whenever P, o or pt change (keys the attention schedule cache)
+  bool in_plan = false;             // between ts_step_plan_prepare and ts_step_plan_commit: no other call may touch it
 };
 
 struct Staging {      // pinned host + device buffer pair for per-call schedule records
@@ -140,6 +157,9 @@ struct ts_pool {
   size_t stage_cap = 0;
   int64_t launches = 0;
   std::vector<int32_t> scratch_mark;       // duplicate detection
+  std::vector<int32_t> scratch_need;       // per-session page demand of the call in progress
+  std::vector<int64_t> scratch_key;        // schedule key of the call in progress
+  std::vector<uint8_t*> retired;           // outgrown staging buffers, freed with the pool (never under running work)
   // attention schedule of the last batch (a1), reused while the batch and its sessions' page tables are unchanged:
   // every layer and denoising pass of one chunk step then pays the scheduler once
   uint64_t ver_seq = 0;                    // source of Session::ver values (never repeats, also across reopen)
@@ -228,7 +248,7 @@ static int check_batch(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
     if (pool->sess[sid].state == TS_SESSION_CLOSED) return TS_ERR_STATE;
   }
   for (int b = 0; b < n; ++b)
-    if (pool->sess[sids[b]].state != TS_SESSION_RESIDENT) return TS_ERR_STATE;
+    if (pool->sess[sids[b]].state != TS_SESSION_RESIDENT || pool->sess[sids[b]].in_plan) return TS_ERR_STATE;
   return TS_OK;
 }
 
@@ -304,7 +324,15 @@ int64_t ts_pool_slab_bytes(const ts_pool_config* cfg) {
 int ts_pool_destroy(ts_pool* pool) {
   if (pool == nullptr) return TS_ERR_INVALID;
   cudaSetDevice(pool->cfg.device);
-  cudaDeviceSynchronize();
+  // wait for the pool's own work only (its streams and the last call recorded on each timeline), not for the device
+  pool->tl_compute.sync_all();
+  pool->tl_side.sync_all();
+  if (pool->side) cudaStreamSynchronize(pool->side);
+  for (cudaStream_t st : {pool->up_s, pool->h2d_s, pool->d2h_s})
+    if (st) cudaStreamSynchronize(st);
+  for (Staging& s : pool->ring)
+    if (s.in_flight && s.ev) cudaEventSynchronize(s.ev);
+  for (uint8_t* r : pool->retired) cudaFree(r);
   for (Staging& s : pool->ring) {
     if (s.h) cudaFreeHost(s.h);
     if (s.d) cudaFree(s.d);
@@ -436,6 +464,7 @@ int ts_session_close(ts_pool* pool, int32_t sid) {
   if (pool == nullptr) return TS_ERR_INVALID;
   if (sid < 0 || sid >= pool->cfg.max_sessions || pool->sess[sid].state == TS_SESSION_CLOSED) return TS_ERR_STATE;
   Session& s = pool->sess[sid];
+  if (s.in_plan) return TS_ERR_STATE;   // a prepared step plan holds it until ts_step_plan_commit
   if (s.state == TS_SESSION_RESIDENT) {
     for (int32_t p : s.pt) {
       pool->page_compute_seq[p] = s.compute_seq;   // in-flight readers/writers of the page
@@ -497,15 +526,342 @@ int ts_pool_stats(ts_pool* pool, ts_pool_stats_t* out) {
 void* ts_pool_side_stream(ts_pool* pool) { return pool ? (void*)pool->side : nullptr; }
 int64_t ts_pool_launch_count(ts_pool* pool) { return pool ? pool->launches : 0; }
 
-// --------------------------------------------------------------------------------------------- attention
+// --------------------------------------------------------------------------------------------- a1: schedule
+// ---- a1: collect + coalesce.  The schedule (session descriptors, packed page tables, cluster work items) depends only
+// on the batch and on its sessions' page-table state, so it is built once and reused by every later call with the same
+// key - all layers and denoising passes of a chunk step.  Result in pool->sched_*.
+static void build_schedule(ts_pool* pool, int32_t n, const int32_t* sids, const int32_t* chunk_frames) {
+  const ts_pool_config& c = pool->cfg;
+  const int T = c.frame_tokens, H = c.n_heads, W = c.window_frames;
+  std::vector<int64_t>& key = pool->scratch_key;
+  key.clear();
+  key.push_back(n);
+  for (int b = 0; b < n; ++b) {
+    key.push_back(sids[b]);
+    key.push_back(chunk_frames[b]);
+    key.push_back((int64_t)pool->sess[sids[b]].ver);
+  }
+  if (key == pool->sched_key) return;
+  const int grid_max = std::max(2, pool->sm_count & ~1);
+  ++pool->sched_builds;
+  std::vector<SessDesc>& sd = pool->sched_sess;
+  std::vector<int32_t>& pt = pool->sched_pt;
+  std::vector<int32_t>& cta_begin = pool->sched_cta;
+  std::vector<WorkItem>& items = pool->sched_items;
+  sd.assign(n, SessDesc());
+  pt.clear();
+  int q_off = 0;
+  for (int b = 0; b < n; ++b) {
+    const Session& s = pool->sess[sids[b]];
+    const int cfr = chunk_frames[b];
+    const int C = cfr * T;
+    const int a = W > 0 ? std::max(0, s.P + cfr - W) : 0;     // window start in frames (R6 i)
+    SessDesc& d = sd[b];
+    d.q_off = q_off;
+    d.C = C;
+    d.x_begin = s.o + a * T;
+    d.x_end = s.o + s.P * T;
+    d.pt_off = (int32_t)pt.size();
+    d.n_pt = (int32_t)s.pt.size();
+    d.pad0 = d.pad1 = 0;
+    pt.insert(pt.end(), s.pt.begin(), s.pt.end());
+    q_off += C;
+  }
+  // Work items come in two granularities: pairs of 128-row query tiles (one K/V tile feeds 256 rows), or single
+  // tiles whose KV tiles alternate between the two TMEM tile slots (half as long, same MMA work per step, twice the
+  // K/V traffic per FLOP).  Pairs are the default; single tiles are taken when the batch is so small that pairs
+  // leave clusters idle in the last wave (1-2 sessions), judged by the modelled makespan of both schedules.
+  struct Cand {
+    int cost, sess, head, q_tile, n_kv;
+    bool single;
+  };
+  struct CItem {
+    int cost;
+    int64_t stream_cost;
+    int stream;
+    Cand a, b;       // b.q_tile < 0: no second item
+    bool mc;
+  };
+  struct Plan {
+    std::vector<CItem> citems;
+    std::vector<std::vector<int>> per_cluster;
+    int64_t makespan = 0;
+  };
+  auto make_plan = [&](int tiles_per_item) {
+    Plan plan;
+    std::vector<Cand> cands;
+    for (int b = 0; b < n; ++b) {
+      const SessDesc& d = sd[b];
+      const int n_tiles = (d.C + 127) / 128;
+      for (int t0 = 0; t0 < n_tiles; t0 += tiles_per_item) {
+        int n_q, n_kv;
+        item_geometry(c, d.C, d.x_begin, d.x_end, t0, tiles_per_item, &n_q, &n_kv);
+        // time model in twentieths of a two-tile KV step, fitted to per-CTA cycle counts on configs[2]
+        // (3184 clk per step + 14.7 k clk per item): 4.5 steps per item for the Q load, pipeline fill and epilogue.
+        // A lone query tile alternates its KV tiles between the two TMEM tile slots (half the steps, plus the merge).
+        const int cost = n_q == 2 ? 20 * n_kv + 90 : (n_kv >= 2 ? 10 * n_kv + 110 : 19 * n_kv + 90);
+        for (int h = 0; h < H; ++h) cands.push_back({cost, b, h, t0, n_kv, tiles_per_item == 1});
+      }
+    }
+    // ---- cluster items.  The items of one (session, head) stream read the same K/V pages: two of them at a time
+    // go to the two CTAs of a cluster, which then load half of every K/V tile each and multicast it to both (mc).
+    // A stream's odd item out is paired with another stream's (or with nothing): those two share a cluster without
+    // sharing loads.  Both CTAs cycle max(n_kv) tiles through their smem rings to stay on the same ring position.
+    std::vector<int64_t> stream_cost((size_t)n * H, 0);
+    for (const Cand& x : cands) stream_cost[(size_t)x.sess * H + x.head] += x.cost;
+    // within a stream: by KV length (longest first), two-tile items before a lone tile
+    std::stable_sort(cands.begin(), cands.end(), [&](const Cand& x, const Cand& y) {
+      const size_t sx = (size_t)x.sess * H + x.head, sy = (size_t)y.sess * H + y.head;
+      if (sx != sy) return sx < sy;
+      if (x.n_kv != y.n_kv) return x.n_kv > y.n_kv;
+      return x.cost > y.cost;
+    });
+    std::vector<CItem>& citems = plan.citems;
+    std::vector<Cand> odd;
+    for (size_t i = 0; i < cands.size();) {
+      size_t e = i;
+      while (e < cands.size() && cands[e].sess == cands[i].sess && cands[e].head == cands[i].head) ++e;
+      const int stream = cands[i].sess * H + cands[i].head;
+      // pair items of EQUAL KV length first (neither CTA then waits for tiles only its partner needs); what is left
+      // over (at most one item per length) is paired in length order, and the stream's last odd item goes to `odd`
+      std::vector<Cand> rest;
+      while (i < e) {
+        if (i + 1 < e && cands[i].n_kv == cands[i + 1].n_kv) {
+          citems.push_back({std::max(cands[i].cost, cands[i + 1].cost), stream_cost[stream], stream, cands[i], cands[i + 1], true});
+          i += 2;
+        } else {
+          rest.push_back(cands[i++]);
+        }
+      }
+      size_t r = 0;
+      for (; r + 1 < rest.size(); r += 2)
+        citems.push_back({std::max(rest[r].cost, rest[r + 1].cost), stream_cost[stream], stream, rest[r], rest[r + 1], true});
+      if (r < rest.size()) odd.push_back(rest[r]);
+    }
+    std::stable_sort(odd.begin(), odd.end(), [](const Cand& x, const Cand& y) { return x.cost > y.cost; });
+    for (size_t i = 0; i < odd.size(); i += 2) {
+      Cand none = odd[i];
+      none.q_tile = -1;
+      none.n_kv = 0;
+      none.cost = 0;
+      const Cand& second = (i + 1 < odd.size()) ? odd[i + 1] : none;
+      const int stream = odd[i].sess * H + odd[i].head;
+      citems.push_back({std::max(odd[i].cost, second.cost), stream_cost[stream], stream, odd[i], second, false});
+    }
+    // List scheduling in stream order, heaviest streams first (LPT at stream granularity, so that the tail of the
+    // schedule is made of short items): a stream's items are dealt out back to back, each to the least-loaded
+    // cluster, and run at the same time - the stream's K/V then comes from DRAM once and from L2 afterwards.
+    std::stable_sort(citems.begin(), citems.end(), [](const CItem& x, const CItem& y) {
+      if (x.stream_cost != y.stream_cost) return x.stream_cost > y.stream_cost;
+      if (x.stream != y.stream) return x.stream < y.stream;
+      return x.cost > y.cost;
+    });
+    const int n_clusters = std::min(grid_max / 2, (int)citems.size());
+    plan.per_cluster.assign(n_clusters, std::vector<int>());
+    typedef std::pair<int64_t, int> Load;   // (load, cluster)
+    std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
+    for (int i = 0; i < n_clusters; ++i) heap.push({0, i});
+    for (int i = 0; i < (int)citems.size(); ++i) {
+      Load top = heap.top();
+      heap.pop();
+      plan.per_cluster[top.second].push_back(i);
+      heap.push({top.first + citems[i].cost, top.second});
+      plan.makespan = std::max(plan.makespan, top.first + citems[i].cost);
+    }
+    return plan;
+  };
+  Plan plan = make_plan(2);
+  if (n * H * 2 <= grid_max) {               // small batch: fewer than two streams per cluster
+    Plan fine = make_plan(1);
+    if (fine.makespan * 108 < plan.makespan * 100) plan = std::move(fine);   // single tiles cost ~8 % more per FLOP
+  }
+  // The kernel hands cluster items out dynamically in THIS order (a global cursor): clusters that run a little
+  // faster simply take more; the list-scheduling above only serves to compare the two plans.
+  items.clear();
+  for (const CItem& it : plan.citems) {
+    for (int r = 0; r < 2; ++r) {
+      const Cand& x = r ? it.b : it.a;
+      WorkItem wi;
+      wi.sess = x.sess;
+      wi.head = x.head;
+      wi.q_tile = x.q_tile;
+      wi.pipe = (uint32_t)std::max(it.a.n_kv, it.b.n_kv) | (it.mc ? 0x80000000u : 0u) | (x.single ? 0x40000000u : 0u);
+      items.push_back(wi);
+    }
+  }
+  cta_begin.assign(1, 2 * (int)plan.per_cluster.size());   // [0] = grid
+  pool->sched_key = key;
+}
+
+// One schedule block: everything a launch reads besides the caller's tensors and the slab, in one piece of (pinned host
+// and, with the same layout, device) memory.  `n_slots` sets of per-session Q/Kn/Vn tensor maps come first.
+struct BlockLayout {
+  size_t off_maps, off_sess, off_pt, off_feed, off_items, off_copy, bytes, feed_bytes;
+};
+
+static BlockLayout block_layout(int n, int n_slots, size_t n_pt, size_t n_items, int grid, bool with_copy) {
+  BlockLayout L;
+  L.feed_bytes = 128 + (size_t)(grid / 2) * kFeedRing * 8;   // header (cursor, end count, n_citems) + per-cluster rings
+  L.off_maps = 0;
+  L.off_sess = align_up(L.off_maps + (size_t)n_slots * n * 3 * sizeof(CUtensorMap), 128);
+  L.off_pt = align_up(L.off_sess + (size_t)n * sizeof(SessDesc), 128);
+  L.off_feed = align_up(L.off_pt + n_pt * 4, 128);
+  L.off_items = align_up(L.off_feed + L.feed_bytes, 128);
+  L.off_copy = align_up(L.off_items + n_items * sizeof(WorkItem), 128);
+  L.bytes = L.off_copy + (with_copy ? (size_t)n * sizeof(CopySess) : 0);
+  return L;
+}
+
+// Everything of the block except the tensor maps, from the pool's current schedule.
+static void fill_block(ts_pool* pool, uint8_t* h, const BlockLayout& L, int n, const CopySess* cs) {
+  memcpy(h + L.off_sess, pool->sched_sess.data(), (size_t)n * sizeof(SessDesc));
+  memcpy(h + L.off_pt, pool->sched_pt.data(), pool->sched_pt.size() * 4);
+  memset(h + L.off_feed, 0, L.feed_bytes);
+  reinterpret_cast<int32_t*>(h + L.off_feed)[2] = (int32_t)(pool->sched_items.size() / 2);
+  memcpy(h + L.off_items, pool->sched_items.data(), pool->sched_items.size() * sizeof(WorkItem));
+  if (cs != nullptr) {
+    CopySess* dst = reinterpret_cast<CopySess*>(h + L.off_copy);
+    for (int b = 0; b < n; ++b) {
+      dst[b] = cs[b];
+      dst[b].pt_off = pool->sched_sess[b].pt_off;   // the append shares the attention's packed page tables
+    }
+  }
+}
+
+// Per-session 3D maps {D, H, C} of the call's packed Q / Kn / Vn: rows past a session's chunk read as zeros, never as a
+// neighbour's tokens.  `chunk_frames` fixes the geometry (q_off, C); nothing else of the schedule is needed.
+static bool encode_session_maps(ts_pool* pool, CUtensorMap* maps, int n, const int32_t* chunk_frames, const void* q,
+                                const void* k, const void* v) {
+  const ts_pool_config& c = pool->cfg;
+  const int H = c.n_heads, D = c.head_dim;
+  size_t q_off = 0;
+  for (int b = 0; b < n; ++b) {
+    const size_t C = (size_t)chunk_frames[b] * c.frame_tokens;
+    const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)H, (cuuint64_t)C};
+    const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)H * D * 2};
+    const cuuint32_t box_q[3] = {64, 1, 128};
+    const cuuint32_t box_kv[3] = {64, 1, (cuuint32_t)std::min(c.page_tokens, 64)};   // same box rows as the cache maps
+    const size_t byte_off = q_off * H * D * 2;
+    if (!encode_map(&maps[b * 3 + 0], (uint8_t*)q + byte_off, 3, dims, strides, box_q)) return false;
+    if (!encode_map(&maps[b * 3 + 1], (uint8_t*)k + byte_off, 3, dims, strides, box_kv)) return false;
+    if (!encode_map(&maps[b * 3 + 2], (uint8_t*)v + byte_off, 3, dims, strides, box_kv)) return false;
+    q_off += C;
+  }
+  return true;
+}
+
+// Kernel parameters of one launch on the block at device address `d` (tensor maps of set `slot`).
+static AttnParams make_params(ts_pool* pool, const BlockLayout& L, uint8_t* d, int n, int slot, int32_t layer, const void* k,
+                              const void* v, void* out, float* lse, float scale, bool with_copy, int total_rows) {
+  const ts_pool_config& c = pool->cfg;
+  AttnParams p;
+  memset(&p.copy, 0, sizeof(p.copy));
+  if (with_copy) {
+    p.copy.sess = reinterpret_cast<const CopySess*>(d + L.off_copy);
+    p.copy.page_tables = reinterpret_cast<const int32_t*>(d + L.off_pt);
+    p.copy.n_sess = n;
+    p.copy.total_rows = total_rows;
+    p.copy.H = c.n_heads;
+    p.copy.D = c.head_dim;
+    p.copy.B = c.page_tokens;
+    p.copy.log2_B = pool->log2_B;
+    p.copy.page_stride = pool->page_bytes;
+    p.copy.layer_k_off = (int64_t)layer * pool->layer_bytes;
+    p.copy.layer_v_off = p.copy.layer_k_off + pool->kv_bytes;
+    p.copy.slab = pool->slab;
+    p.copy.src_k = (const uint8_t*)k;
+    p.copy.src_v = (const uint8_t*)v;
+  }
+  p.map_k = pool->map_k[layer];
+  p.map_v = pool->map_v[layer];
+  p.sess_maps = reinterpret_cast<const CUtensorMap*>(d + L.off_maps) + (size_t)slot * n * 3;
+  p.sess = reinterpret_cast<const SessDesc*>(d + L.off_sess);
+  p.page_tables = reinterpret_cast<const int32_t*>(d + L.off_pt);
+  p.feed_hdr = reinterpret_cast<int32_t*>(d + L.off_feed);
+  p.feed = reinterpret_cast<unsigned long long*>(d + L.off_feed + 128);
+  p.items = reinterpret_cast<const WorkItem*>(d + L.off_items);
+  p.out = (uint16_t*)out;
+  p.lse = lse;
+  p.H = c.n_heads;
+  p.T = c.frame_tokens;
+  p.B = c.page_tokens;
+  p.log2_B = pool->log2_B;
+  p.scale = scale;
+  p.scale_log2 = scale * 1.4426950408889634f;
+  return p;
+}
+
+// Page demand of appending the batch's chunks (O2: max(0, ceil((o + L + C) / B) - |PT|) per session, R14).
+// Returns the total, the per-session demand in pool->scratch_need.
+static int64_t page_demand(ts_pool* pool, int32_t n, const int32_t* sids, const int32_t* chunk_frames) {
+  const int T = pool->cfg.frame_tokens, B = pool->cfg.page_tokens;
+  pool->scratch_need.assign(n, 0);
+  int64_t total = 0;
+  for (int b = 0; b < n; ++b) {
+    const Session& s = pool->sess[sids[b]];
+    const int64_t end = (int64_t)s.o + (int64_t)s.P * T + (int64_t)chunk_frames[b] * T;
+    pool->scratch_need[b] = (int)std::max<int64_t>(0, (end + B - 1) / B - (int64_t)s.pt.size());
+    total += pool->scratch_need[b];
+  }
+  return total;
+}
+
 // The KV append of a fused chunk step, prepared on the host (pages already allocated) and carried out by the idle
 // warps of the attention kernel.
 struct FusedAppend {
   std::vector<CopySess> cs;            // pt_off is filled in from the attention schedule (same packed page tables)
   uint64_t wait_side = 0, wait_compute = 0;
   int total_rows = 0;
+  std::vector<int32_t> popped;         // page ids taken from the free list, in pop order (rolled back on failure)
 };
 
+// Grows the page tables of the batch by pool->scratch_need (popping from the front of the free list, sessions in `sids`
+// order) and describes the append of the chunks that follows.  The caller has checked the demand against the free list.
+static void grow_for_append(ts_pool* pool, int32_t n, const int32_t* sids, const int32_t* chunk_frames, FusedAppend* fa) {
+  const int T = pool->cfg.frame_tokens, B = pool->cfg.page_tokens;
+  fa->cs.resize(n);
+  int tok_off = 0, row_off = 0;
+  for (int b = 0; b < n; ++b) {
+    Session& s = pool->sess[sids[b]];
+    const int need = pool->scratch_need[b];
+    if (need > 0) s.ver = ++pool->ver_seq;
+    for (int i = 0; i < need; ++i) {
+      const int32_t pg = pool->free_q.front();
+      pool->free_q.pop_front();
+      fa->wait_side = std::max(fa->wait_side, pool->page_side_seq[pg]);        // a D2H copy out of the page may be pending
+      fa->wait_compute = std::max(fa->wait_compute, pool->page_compute_seq[pg]);
+      s.pt.push_back(pg);
+      fa->popped.push_back(pg);
+    }
+    fa->wait_side = std::max(fa->wait_side, s.side_seq);
+    const int C = chunk_frames[b] * T;
+    const int x0 = s.o + s.P * T;
+    CopySess& d = fa->cs[b];
+    d.tok_off = tok_off;
+    d.n_tok = C;
+    d.n_zero = (B - ((x0 + C) & (B - 1))) & (B - 1);
+    d.x0 = x0;
+    d.pt_off = 0;
+    d.row_off = row_off;
+    d.pad0 = d.pad1 = 0;
+    tok_off += C;
+    row_off += d.n_tok + d.n_zero;
+  }
+  fa->total_rows = row_off;
+}
+
+// Undoes grow_for_append after a failure further down (all-or-nothing): the popped ids go back to the FRONT of the free
+// list in their original order and leave the tables they were appended to.
+static void ungrow(ts_pool* pool, int32_t n, const int32_t* sids, const FusedAppend& fa) {
+  for (int b = n - 1; b >= 0; --b) {
+    Session& s = pool->sess[sids[b]];
+    for (int i = 0; i < pool->scratch_need[b]; ++i) s.pt.pop_back();
+    if (pool->scratch_need[b] > 0) s.ver = ++pool->ver_seq;
+  }
+  for (auto it = fa.popped.rbegin(); it != fa.popped.rend(); ++it) pool->free_q.push_front(*it);
+}
+
+// --------------------------------------------------------------------------------------------- attention
 static int attention_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
                           const void* q, const void* k, const void* v, void* out, float* lse, float scale,
                           void* cuda_stream, const FusedAppend* fused, uint64_t* seq_out) {
@@ -519,210 +875,15 @@ static int attention_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t
   const ts_pool_config& c = pool->cfg;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   TS_CUDA(cudaSetDevice(c.device));
-  const int T = c.frame_tokens, H = c.n_heads, D = c.head_dim, W = c.window_frames;
 
-  // ---- a1: collect + coalesce.  The schedule (session descriptors, packed page tables, work items per CTA) depends
-  // only on the batch and on its sessions' page-table state, so it is built once and reused by every later call with
-  // the same key - all layers and denoising passes of a chunk step; only the Q/K/V tensor maps are encoded per call.
-  std::vector<int64_t> key;
-  key.reserve(3 * (size_t)n + 1);
-  key.push_back(n);
-  for (int b = 0; b < n; ++b) {
-    key.push_back(sids[b]);
-    key.push_back(chunk_frames[b]);
-    key.push_back((int64_t)pool->sess[sids[b]].ver);
-  }
-  const int grid_max = std::max(2, pool->sm_count & ~1);
-  if (key != pool->sched_key) {
-    ++pool->sched_builds;
-    std::vector<SessDesc>& sd = pool->sched_sess;
-    std::vector<int32_t>& pt = pool->sched_pt;
-    std::vector<int32_t>& cta_begin = pool->sched_cta;
-    std::vector<WorkItem>& items = pool->sched_items;
-    sd.assign(n, SessDesc());
-    pt.clear();
-    int q_off = 0;
-    for (int b = 0; b < n; ++b) {
-      const Session& s = pool->sess[sids[b]];
-      const int cfr = chunk_frames[b];
-      const int C = cfr * T;
-      const int a = W > 0 ? std::max(0, s.P + cfr - W) : 0;     // window start in frames (R6 i)
-      SessDesc& d = sd[b];
-      d.q_off = q_off;
-      d.C = C;
-      d.x_begin = s.o + a * T;
-      d.x_end = s.o + s.P * T;
-      d.pt_off = (int32_t)pt.size();
-      d.n_pt = (int32_t)s.pt.size();
-      d.pad0 = d.pad1 = 0;
-      pt.insert(pt.end(), s.pt.begin(), s.pt.end());
-      q_off += C;
-    }
-    // Work items come in two granularities: pairs of 128-row query tiles (one K/V tile feeds 256 rows), or single
-    // tiles whose KV tiles alternate between the two TMEM tile slots (half as long, same MMA work per step, twice the
-    // K/V traffic per FLOP).  Pairs are the default; single tiles are taken when the batch is so small that pairs
-    // leave clusters idle in the last wave (1-2 sessions), judged by the modelled makespan of both schedules.
-    struct Cand {
-      int cost, sess, head, q_tile, n_kv;
-      bool single;
-    };
-    struct CItem {
-      int cost;
-      int64_t stream_cost;
-      int stream;
-      Cand a, b;       // b.q_tile < 0: no second item
-      bool mc;
-    };
-    struct Plan {
-      std::vector<CItem> citems;
-      std::vector<std::vector<int>> per_cluster;
-      int64_t makespan = 0;
-    };
-    auto make_plan = [&](int tiles_per_item) {
-      Plan plan;
-      std::vector<Cand> cands;
-      for (int b = 0; b < n; ++b) {
-        const SessDesc& d = sd[b];
-        const int n_tiles = (d.C + 127) / 128;
-        for (int t0 = 0; t0 < n_tiles; t0 += tiles_per_item) {
-          int n_q, n_kv;
-          item_geometry(c, d.C, d.x_begin, d.x_end, t0, tiles_per_item, &n_q, &n_kv);
-          // time model in twentieths of a two-tile KV step, fitted to per-CTA cycle counts on configs[2]
-          // (3184 clk per step + 14.7 k clk per item): 4.5 steps per item for the Q load, pipeline fill and epilogue.
-          // A lone query tile alternates its KV tiles between the two TMEM tile slots (half the steps, plus the merge).
-          const int cost = n_q == 2 ? 20 * n_kv + 90 : (n_kv >= 2 ? 10 * n_kv + 110 : 19 * n_kv + 90);
-          for (int h = 0; h < H; ++h) cands.push_back({cost, b, h, t0, n_kv, tiles_per_item == 1});
-        }
-      }
-      // ---- cluster items.  The items of one (session, head) stream read the same K/V pages: two of them at a time
-      // go to the two CTAs of a cluster, which then load half of every K/V tile each and multicast it to both (mc).
-      // A stream's odd item out is paired with another stream's (or with nothing): those two share a cluster without
-      // sharing loads.  Both CTAs cycle max(n_kv) tiles through their smem rings to stay on the same ring position.
-      std::vector<int64_t> stream_cost((size_t)n * H, 0);
-      for (const Cand& x : cands) stream_cost[(size_t)x.sess * H + x.head] += x.cost;
-      // within a stream: by KV length (longest first), two-tile items before a lone tile
-      std::stable_sort(cands.begin(), cands.end(), [&](const Cand& x, const Cand& y) {
-        const size_t sx = (size_t)x.sess * H + x.head, sy = (size_t)y.sess * H + y.head;
-        if (sx != sy) return sx < sy;
-        if (x.n_kv != y.n_kv) return x.n_kv > y.n_kv;
-        return x.cost > y.cost;
-      });
-      std::vector<CItem>& citems = plan.citems;
-      std::vector<Cand> odd;
-      for (size_t i = 0; i < cands.size();) {
-        size_t e = i;
-        while (e < cands.size() && cands[e].sess == cands[i].sess && cands[e].head == cands[i].head) ++e;
-        const int stream = cands[i].sess * H + cands[i].head;
-        // pair items of EQUAL KV length first (neither CTA then waits for tiles only its partner needs); what is left
-        // over (at most one item per length) is paired in length order, and the stream's last odd item goes to `odd`
-        std::vector<Cand> rest;
-        while (i < e) {
-          if (i + 1 < e && cands[i].n_kv == cands[i + 1].n_kv) {
-            citems.push_back({std::max(cands[i].cost, cands[i + 1].cost), stream_cost[stream], stream, cands[i], cands[i + 1], true});
-            i += 2;
-          } else {
-            rest.push_back(cands[i++]);
-          }
-        }
-        size_t r = 0;
-        for (; r + 1 < rest.size(); r += 2)
-          citems.push_back({std::max(rest[r].cost, rest[r + 1].cost), stream_cost[stream], stream, rest[r], rest[r + 1], true});
-        if (r < rest.size()) odd.push_back(rest[r]);
-      }
-      std::stable_sort(odd.begin(), odd.end(), [](const Cand& x, const Cand& y) { return x.cost > y.cost; });
-      for (size_t i = 0; i < odd.size(); i += 2) {
-        Cand none = odd[i];
-        none.q_tile = -1;
-        none.n_kv = 0;
-        none.cost = 0;
-        const Cand& second = (i + 1 < odd.size()) ? odd[i + 1] : none;
-        const int stream = odd[i].sess * H + odd[i].head;
-        citems.push_back({std::max(odd[i].cost, second.cost), stream_cost[stream], stream, odd[i], second, false});
-      }
-      // List scheduling in stream order, heaviest streams first (LPT at stream granularity, so that the tail of the
-      // schedule is made of short items): a stream's items are dealt out back to back, each to the least-loaded
-      // cluster, and run at the same time - the stream's K/V then comes from DRAM once and from L2 afterwards.
-      std::stable_sort(citems.begin(), citems.end(), [](const CItem& x, const CItem& y) {
-        if (x.stream_cost != y.stream_cost) return x.stream_cost > y.stream_cost;
-        if (x.stream != y.stream) return x.stream < y.stream;
-        return x.cost > y.cost;
-      });
-      const int n_clusters = std::min(grid_max / 2, (int)citems.size());
-      plan.per_cluster.assign(n_clusters, std::vector<int>());
-      typedef std::pair<int64_t, int> Load;   // (load, cluster)
-      std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
-      for (int i = 0; i < n_clusters; ++i) heap.push({0, i});
-      for (int i = 0; i < (int)citems.size(); ++i) {
-        Load top = heap.top();
-        heap.pop();
-        plan.per_cluster[top.second].push_back(i);
-        heap.push({top.first + citems[i].cost, top.second});
-        plan.makespan = std::max(plan.makespan, top.first + citems[i].cost);
-      }
-      return plan;
-    };
-    Plan plan = make_plan(2);
-    if (n * H * 2 <= grid_max) {               // small batch: fewer than two streams per cluster
-      Plan fine = make_plan(1);
-      if (fine.makespan * 108 < plan.makespan * 100) plan = std::move(fine);   // single tiles cost ~8 % more per FLOP
-    }
-    // The kernel hands cluster items out dynamically in THIS order (a global cursor): clusters that run a little
-    // faster simply take more; the list-scheduling above only serves to compare the two plans.
-    items.clear();
-    for (const CItem& it : plan.citems) {
-      for (int r = 0; r < 2; ++r) {
-        const Cand& x = r ? it.b : it.a;
-        WorkItem wi;
-        wi.sess = x.sess;
-        wi.head = x.head;
-        wi.q_tile = x.q_tile;
-        wi.pipe = (uint32_t)std::max(it.a.n_kv, it.b.n_kv) | (it.mc ? 0x80000000u : 0u) | (x.single ? 0x40000000u : 0u);
-        items.push_back(wi);
-      }
-    }
-    cta_begin.assign(1, 2 * (int)plan.per_cluster.size());   // [0] = grid
-    pool->sched_key = key;
-  }
+  build_schedule(pool, n, sids, chunk_frames);
   const int grid = pool->sched_cta[0];
-  const int n_citems = (int)pool->sched_items.size() / 2;
-  const size_t feed_bytes = 128 + (size_t)(grid / 2) * kFeedRing * 8;   // cursor + per-cluster rings, zeroed per call
-  ScheduleLayout L;
-  L.n_items = (int)pool->sched_items.size();
-  L.grid = grid;
-  L.off_maps = 0;
-  L.off_sess = align_up(L.off_maps + (size_t)n * 3 * sizeof(CUtensorMap), 128);
-  L.off_pt = align_up(L.off_sess + (size_t)n * sizeof(SessDesc), 128);
-  L.off_cta = align_up(L.off_pt + pool->sched_pt.size() * 4, 128);
-  L.off_items = align_up(L.off_cta + feed_bytes, 128);
-  const size_t off_copy = align_up(L.off_items + pool->sched_items.size() * sizeof(WorkItem), 128);
-  L.bytes = off_copy + (fused ? (size_t)n * sizeof(CopySess) : 0);
+  const BlockLayout L = block_layout(n, 1, pool->sched_pt.size(), pool->sched_items.size(), grid, fused != nullptr);
   Staging* st = nullptr;
   rc = acquire_staging(pool, L.bytes, &st);
   if (rc != TS_OK) return rc;
-  CUtensorMap* maps = reinterpret_cast<CUtensorMap*>(st->h + L.off_maps);
-  memcpy(st->h + L.off_sess, pool->sched_sess.data(), (size_t)n * sizeof(SessDesc));
-  memcpy(st->h + L.off_pt, pool->sched_pt.data(), pool->sched_pt.size() * 4);
-  memset(st->h + L.off_cta, 0, feed_bytes);
-  memcpy(st->h + L.off_items, pool->sched_items.data(), pool->sched_items.size() * sizeof(WorkItem));
-  if (fused) {
-    CopySess* cs = reinterpret_cast<CopySess*>(st->h + off_copy);
-    for (int b = 0; b < n; ++b) {
-      cs[b] = fused->cs[b];
-      cs[b].pt_off = pool->sched_sess[b].pt_off;
-    }
-  }
-  for (int b = 0; b < n; ++b) {
-    // per-session 3D maps {D, H, C}: rows past the session's chunk read as zeros, never as a neighbour's tokens
-    const SessDesc& d = pool->sched_sess[b];
-    const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)H, (cuuint64_t)d.C};
-    const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)H * D * 2};
-    const cuuint32_t box_q[3] = {64, 1, 128};
-    const cuuint32_t box_kv[3] = {64, 1, (cuuint32_t)std::min(c.page_tokens, 64)};   // same box rows as the cache maps
-    const size_t byte_off = (size_t)d.q_off * H * D * 2;
-    if (!encode_map(&maps[b * 3 + 0], (uint8_t*)q + byte_off, 3, dims, strides, box_q)) return TS_ERR_CUDA;
-    if (!encode_map(&maps[b * 3 + 1], (uint8_t*)k + byte_off, 3, dims, strides, box_kv)) return TS_ERR_CUDA;
-    if (!encode_map(&maps[b * 3 + 2], (uint8_t*)v + byte_off, 3, dims, strides, box_kv)) return TS_ERR_CUDA;
-  }
+  fill_block(pool, st->h, L, n, fused ? fused->cs.data() : nullptr);
+  if (!encode_session_maps(pool, reinterpret_cast<CUtensorMap*>(st->h + L.off_maps), n, chunk_frames, q, k, v)) return TS_ERR_CUDA;
 
   // ---- ordering: wait (stream-side) for pending resumes of the batch's sessions
   for (int b = 0; b < n; ++b) TS_CUDA(pool->tl_side.wait(stream, pool->sess[sids[b]].side_seq));
@@ -733,42 +894,9 @@ static int attention_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t
 
   rc = upload_staging(pool, st, L.bytes, stream);
   if (rc != TS_OK) return rc;
-  AttnParams p;
-  memset(&p.copy, 0, sizeof(p.copy));
-  if (fused) {
-    p.copy.sess = reinterpret_cast<const CopySess*>(st->d + off_copy);
-    p.copy.page_tables = reinterpret_cast<const int32_t*>(st->d + L.off_pt);
-    p.copy.n_sess = n;
-    p.copy.total_rows = fused->total_rows;
-    p.copy.H = H;
-    p.copy.D = D;
-    p.copy.B = c.page_tokens;
-    p.copy.log2_B = pool->log2_B;
-    p.copy.page_stride = pool->page_bytes;
-    p.copy.layer_k_off = (int64_t)layer * pool->layer_bytes;
-    p.copy.layer_v_off = p.copy.layer_k_off + pool->kv_bytes;
-    p.copy.slab = pool->slab;
-    p.copy.src_k = (const uint8_t*)k;
-    p.copy.src_v = (const uint8_t*)v;
-  }
-  p.map_k = pool->map_k[layer];
-  p.map_v = pool->map_v[layer];
-  p.sess_maps = reinterpret_cast<const CUtensorMap*>(st->d + L.off_maps);
-  p.sess = reinterpret_cast<const SessDesc*>(st->d + L.off_sess);
-  p.page_tables = reinterpret_cast<const int32_t*>(st->d + L.off_pt);
-  p.feed_counter = reinterpret_cast<int32_t*>(st->d + L.off_cta);
-  p.feed = reinterpret_cast<unsigned long long*>(st->d + L.off_cta + 128);
-  p.n_citems = n_citems;
-  p.items = reinterpret_cast<const WorkItem*>(st->d + L.off_items);
-  p.out = (uint16_t*)out;
-  p.lse = lse;
-  p.H = H;
-  p.T = T;
-  p.B = c.page_tokens;
-  p.log2_B = pool->log2_B;
-  p.scale = scale;
-  p.scale_log2 = scale * 1.4426950408889634f;
-  TS_CUDA(launch_attention(p, D, grid, stream));
+  const AttnParams p = make_params(pool, L, st->d, n, 0, layer, k, v, out, lse, scale, fused != nullptr,
+                                   fused ? fused->total_rows : 0);
+  TS_CUDA(launch_attention(p, c.head_dim, grid, stream));
   ++pool->launches;
   TS_CUDA(cudaEventRecord(st->ev, stream));
   st->in_flight = true;
@@ -915,53 +1043,210 @@ int ts_chunk_step(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, 
   if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) != 0) return TS_ERR_INVALID;
   if (!(scale > 0.0f) || !std::isfinite(scale)) return TS_ERR_INVALID;
   if ((flags & ~(uint32_t)TS_COMMIT) != 0) return TS_ERR_INVALID;
-  const int T = pool->cfg.frame_tokens, B = pool->cfg.page_tokens;
   // page demand of the append, before anything changes or is enqueued (all-or-nothing, O2)
-  std::vector<int> need(n);
-  int64_t need_total = 0;
-  for (int b = 0; b < n; ++b) {
-    const Session& s = pool->sess[sids[b]];
-    const int64_t end = (int64_t)s.o + (int64_t)s.P * T + (int64_t)chunk_frames[b] * T;
-    need[b] = (int)std::max<int64_t>(0, (end + B - 1) / B - (int64_t)s.pt.size());
-    need_total += need[b];
-  }
-  if (need_total > (int64_t)pool->free_q.size()) return TS_ERR_NO_PAGES;
+  if (page_demand(pool, n, sids, chunk_frames) > (int64_t)pool->free_q.size()) return TS_ERR_NO_PAGES;
   // grow the page tables first: the attention schedule is then built from the grown tables (the attention itself only
   // reads [x_begin, x_end), R5) and its packed page-table array also serves the append, which the idle warps of the
   // attention kernel carry out - it is HBM-bound, the attention is not, so it costs the step nothing there
   FusedAppend fa;
-  fa.cs.resize(n);
-  int tok_off = 0, row_off = 0;
-  for (int b = 0; b < n; ++b) {
-    Session& s = pool->sess[sids[b]];
-    if (need[b] > 0) s.ver = ++pool->ver_seq;
-    for (int i = 0; i < need[b]; ++i) {
-      const int32_t pg = pool->free_q.front();
-      pool->free_q.pop_front();
-      fa.wait_side = std::max(fa.wait_side, pool->page_side_seq[pg]);        // a D2H copy out of the page may be pending
-      fa.wait_compute = std::max(fa.wait_compute, pool->page_compute_seq[pg]);
-      s.pt.push_back(pg);
-    }
-    const int C = chunk_frames[b] * T;
-    const int x0 = s.o + s.P * T;
-    CopySess& d = fa.cs[b];
-    d.tok_off = tok_off;
-    d.n_tok = C;
-    d.n_zero = (B - ((x0 + C) & (B - 1))) & (B - 1);
-    d.x0 = x0;
-    d.pt_off = 0;
-    d.row_off = row_off;
-    d.pad0 = d.pad1 = 0;
-    tok_off += C;
-    row_off += d.n_tok + d.n_zero;
-  }
-  fa.total_rows = row_off;
+  grow_for_append(pool, n, sids, chunk_frames, &fa);
   uint64_t seq = 0;
   rc = attention_impl(pool, layer, n, sids, chunk_frames, q, k, v, out, lse, scale, cuda_stream, &fa, &seq);
-  if (rc != TS_OK) return rc;
+  if (rc != TS_OK) {
+    ungrow(pool, n, sids, fa);   // a CUDA failure on the way: the tables and the free list are as before the call
+    return rc;
+  }
   append_commit(pool, n, sids, chunk_frames, flags, seq);
   return TS_OK;
 }
+
+// --------------------------------------------------------------------------------------------- step plan (capture-safe)
+}  // extern "C"
+
+struct ts_step_plan {
+  ts_pool* pool = nullptr;
+  int n = 0, n_slots = 0, grid = 0;
+  std::vector<int32_t> sids, cf;
+  struct Slot {
+    const void *q = nullptr, *k = nullptr, *v = nullptr;
+    void* out = nullptr;
+    float* lse = nullptr;
+    bool bound = false;
+  };
+  std::vector<Slot> slots;
+  std::vector<CUtensorMap> maps;     // [n_slots][n][3], encoded at bind time
+  BlockLayout L;                     // fixed at creation for the largest page tables / item lists the batch can have
+  size_t max_pt = 0, max_items = 0;
+  uint8_t* d = nullptr;              // device block: its address never changes, so captured launches stay valid
+  uint8_t* h[2] = {nullptr, nullptr};
+  cudaEvent_t h_ev[2] = {nullptr, nullptr};
+  bool h_busy[2] = {false, false};
+  int h_next = 0;
+  bool prepared = false;
+  int total_rows = 0;
+  int64_t prepares = 0;
+};
+
+extern "C" {
+
+int ts_step_plan_destroy(ts_step_plan* plan) {
+  if (plan == nullptr) return TS_ERR_INVALID;
+  ts_pool* pool = plan->pool;
+  cudaSetDevice(pool->cfg.device);
+  if (plan->prepared)
+    for (int32_t sid : plan->sids) pool->sess[sid].in_plan = false;
+  for (int i = 0; i < 2; ++i) {
+    if (plan->h_ev[i]) {
+      if (plan->h_busy[i]) cudaEventSynchronize(plan->h_ev[i]);
+      cudaEventDestroy(plan->h_ev[i]);
+    }
+    if (plan->h[i]) cudaFreeHost(plan->h[i]);
+  }
+  if (plan->d) cudaFree(plan->d);   // (synchronises with launches still reading the block)
+  cudaGetLastError();
+  delete plan;
+  return TS_OK;
+}
+
+int ts_step_plan_create(ts_pool* pool, int32_t n, const int32_t* sids, const int32_t* chunk_frames, int32_t n_slots,
+                        ts_step_plan** out) {
+  if (pool == nullptr || out == nullptr) return TS_ERR_INVALID;
+  *out = nullptr;
+  if (n < 1 || n_slots < 1 || n_slots > 4096) return TS_ERR_INVALID;
+  int rc = check_batch(pool, 0, n, sids, chunk_frames);
+  if (rc != TS_OK) return rc;
+  const ts_pool_config& c = pool->cfg;
+  TS_CUDA(cudaSetDevice(c.device));
+  ts_step_plan* plan = new ts_step_plan();
+  plan->pool = pool;
+  plan->n = n;
+  plan->n_slots = n_slots;
+  plan->sids.assign(sids, sids + n);
+  plan->cf.assign(chunk_frames, chunk_frames + n);
+  plan->slots.resize(n_slots);
+  plan->maps.resize((size_t)n_slots * n * 3);
+  plan->grid = std::max(2, pool->sm_count & ~1);   // always the full grid: the launch configuration never changes
+  // upper bounds that hold for every state the batch's sessions can be in: a table holds at most o + (W + c) T tokens
+  // (all of the pool without a window), and a stream of t query tiles makes at most t cluster items (2 t work items)
+  const int64_t T = c.frame_tokens, B = c.page_tokens;
+  for (int b = 0; b < n; ++b) {
+    int64_t pages = c.n_pages;
+    if (c.window_frames > 0)
+      pages = std::min<int64_t>(pages, (B - 1 + ((int64_t)c.window_frames + chunk_frames[b]) * T + B - 1) / B + 1);
+    plan->max_pt += (size_t)pages;
+    const int64_t tiles = ((int64_t)chunk_frames[b] * T + 127) / 128;
+    plan->max_items += (size_t)(2 * tiles * c.n_heads);
+  }
+  plan->L = block_layout(n, n_slots, plan->max_pt, plan->max_items, plan->grid, true);
+  auto fail = [&](int code) {
+    ts_step_plan_destroy(plan);
+    return code;
+  };
+  if (!cuda_ok(cudaMalloc((void**)&plan->d, plan->L.bytes), "cudaMalloc(step plan)")) return fail(TS_ERR_CUDA);
+  if (!cuda_ok(cudaMemset(plan->d, 0, plan->L.bytes), "cudaMemset(step plan)")) return fail(TS_ERR_CUDA);
+  for (int i = 0; i < 2; ++i) {
+    if (!cuda_ok(cudaHostAlloc((void**)&plan->h[i], plan->L.bytes, cudaHostAllocDefault), "cudaHostAlloc(step plan)"))
+      return fail(TS_ERR_CUDA);
+    if (!cuda_ok(cudaEventCreateWithFlags(&plan->h_ev[i], cudaEventDisableTiming), "cudaEventCreate")) return fail(TS_ERR_CUDA);
+  }
+  if (!cuda_ok(attention_configure(c.head_dim), "cudaFuncSetAttribute(attention)")) return fail(TS_ERR_CUDA);
+  *out = plan;
+  return TS_OK;
+}
+
+int ts_step_plan_bind(ts_step_plan* plan, int32_t slot, const void* q, const void* k, const void* v, void* out, float* lse) {
+  if (plan == nullptr || slot < 0 || slot >= plan->n_slots) return TS_ERR_INVALID;
+  if (q == nullptr || k == nullptr || v == nullptr || out == nullptr) return TS_ERR_INVALID;
+  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) != 0) return TS_ERR_INVALID;
+  if (plan->prepared) return TS_ERR_STATE;   // the maps travel with the prepare upload
+  if (!encode_session_maps(plan->pool, plan->maps.data() + (size_t)slot * plan->n * 3, plan->n, plan->cf.data(), q, k, v))
+    return TS_ERR_CUDA;
+  ts_step_plan::Slot& s = plan->slots[slot];
+  s.q = q;
+  s.k = k;
+  s.v = v;
+  s.out = out;
+  s.lse = lse;
+  s.bound = true;
+  return TS_OK;
+}
+
+int ts_step_plan_prepare(ts_step_plan* plan, void* cuda_stream) {
+  if (plan == nullptr) return TS_ERR_INVALID;
+  if (plan->prepared) return TS_ERR_STATE;
+  ts_pool* pool = plan->pool;
+  const int n = plan->n;
+  const int32_t* sids = plan->sids.data();
+  const int32_t* cf = plan->cf.data();
+  int rc = check_batch(pool, 0, n, sids, cf);
+  if (rc != TS_OK) return rc;
+  if (page_demand(pool, n, sids, cf) > (int64_t)pool->free_q.size()) return TS_ERR_NO_PAGES;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  TS_CUDA(cudaSetDevice(pool->cfg.device));
+  const int slot = plan->h_next;
+  if (plan->h_busy[slot]) {           // the upload two prepares ago: long done
+    TS_CUDA(cudaEventSynchronize(plan->h_ev[slot]));
+    plan->h_busy[slot] = false;
+  }
+  FusedAppend fa;
+  grow_for_append(pool, n, sids, cf, &fa);
+  build_schedule(pool, n, sids, cf);
+  if (pool->sched_pt.size() > plan->max_pt || pool->sched_items.size() > plan->max_items) {   // cannot happen: bounds above
+    ungrow(pool, n, sids, fa);
+    return TS_ERR_INVALID;
+  }
+  uint8_t* h = plan->h[slot];
+  fill_block(pool, h, plan->L, n, fa.cs.data());
+  memcpy(h + plan->L.off_maps, plan->maps.data(), plan->maps.size() * sizeof(CUtensorMap));
+  // ordering, all stream-side: pending resumes of the batch, copies out of / readers of the pages the append will write
+  cudaError_t e = cudaSuccess;
+  for (int b = 0; b < n && e == cudaSuccess; ++b) e = pool->tl_side.wait(stream, pool->sess[sids[b]].side_seq);
+  if (e == cudaSuccess) e = pool->tl_side.wait(stream, fa.wait_side);
+  if (e == cudaSuccess) e = pool->tl_compute.wait(stream, fa.wait_compute);
+  // the block is rewritten in stream order: after the previous step's launches, before this step's
+  if (e == cudaSuccess) e = cudaMemcpyAsync(plan->d, h, plan->L.bytes, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess) e = cudaEventRecord(plan->h_ev[slot], stream);
+  if (!cuda_ok(e, "ts_step_plan_prepare")) {
+    ungrow(pool, n, sids, fa);
+    return TS_ERR_CUDA;
+  }
+  plan->h_busy[slot] = true;
+  plan->h_next ^= 1;
+  plan->total_rows = fa.total_rows;
+  plan->prepared = true;
+  ++plan->prepares;
+  for (int b = 0; b < n; ++b) pool->sess[sids[b]].in_plan = true;
+  return TS_OK;
+}
+
+int ts_step_plan_run(ts_step_plan* plan, int32_t layer, int32_t slot, float scale, uint32_t run_flags, void* cuda_stream) {
+  if (plan == nullptr) return TS_ERR_INVALID;
+  ts_pool* pool = plan->pool;
+  if (layer < 0 || layer >= pool->cfg.n_layers || slot < 0 || slot >= plan->n_slots) return TS_ERR_INVALID;
+  if ((run_flags & ~(uint32_t)TS_RUN_APPEND) != 0 || !(scale > 0.0f) || !std::isfinite(scale)) return TS_ERR_INVALID;
+  if (!plan->prepared || !plan->slots[slot].bound) return TS_ERR_STATE;
+  const ts_step_plan::Slot& s = plan->slots[slot];
+  const bool with_copy = (run_flags & TS_RUN_APPEND) != 0;
+  const AttnParams p = make_params(pool, plan->L, plan->d, plan->n, slot, layer, s.k, s.v, s.out, s.lse, scale, with_copy,
+                                   plan->total_rows);
+  TS_CUDA(launch_attention(p, pool->cfg.head_dim, plan->grid, (cudaStream_t)cuda_stream));   // the only stream operation
+  ++pool->launches;
+  return TS_OK;
+}
+
+int ts_step_plan_commit(ts_step_plan* plan, uint32_t flags, void* cuda_stream) {
+  if (plan == nullptr || (flags & ~(uint32_t)TS_COMMIT) != 0) return TS_ERR_INVALID;
+  if (!plan->prepared) return TS_ERR_STATE;
+  ts_pool* pool = plan->pool;
+  TS_CUDA(cudaSetDevice(pool->cfg.device));
+  const uint64_t seq = pool->tl_compute.record((cudaStream_t)cuda_stream);   // after every launch of the step
+  for (int32_t sid : plan->sids) pool->sess[sid].in_plan = false;
+  append_commit(pool, plan->n, plan->sids.data(), plan->cf.data(), flags, seq);
+  plan->prepared = false;
+  return TS_OK;
+}
+
+int64_t ts_step_plan_block_bytes(ts_step_plan* plan) { return plan ? (int64_t)plan->L.bytes : 0; }
 
 // --------------------------------------------------------------------------------------------- gather
 int ts_gather_kv(ts_pool* pool, int32_t layer, int32_t sid, void* k_out, void* v_out, void* cuda_stream) {
@@ -1040,6 +1325,7 @@ int ts_session_suspend(ts_pool* pool, int32_t sid) {
   const ts_pool_config& c = pool->cfg;
   if (sid < 0 || sid >= c.max_sessions || pool->sess[sid].state != TS_SESSION_RESIDENT) return TS_ERR_STATE;
   Session& s = pool->sess[sid];
+  if (s.in_plan) return TS_ERR_STATE;   // chunk-boundary rule (R12): not inside a prepared step
   if (s.pt.size() > pool->host_free.size()) return TS_ERR_NO_HOST;
   TS_CUDA(cudaSetDevice(c.device));
   // chunk-boundary rule (R12): the copy out starts after the compute work already enqueued on the session
@@ -1102,7 +1388,7 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
       a.frame_tokens != b.frame_tokens || a.window_frames != b.window_frames)
     return TS_ERR_INVALID;
   Session& s = src->sess[sid];
-  if (s.state != TS_SESSION_RESIDENT) return TS_ERR_STATE;   // (i): only a live, frozen state moves
+  if (s.state != TS_SESSION_RESIDENT || s.in_plan) return TS_ERR_STATE;   // (i): only a live, frozen state moves
   int new_sid = -1;
   for (int i = 0; i < b.max_sessions && new_sid < 0; ++i)
     if (dst->sess[i].state == TS_SESSION_CLOSED) new_sid = i;
@@ -1126,7 +1412,7 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
     const int rc = acquire_staging(dst, n * 8, &st);
     if (rc != TS_OK) return rc;
   }
-  // ---- nothing can fail for a reason of ours from here on: install on the target (as a resume would)
+  // ---- install on the target (as a resume would); a CUDA failure below puts the popped ids back (nothing changes)
   Session& t = dst->sess[new_sid];
   t = Session();
   t.P = s.P;
@@ -1138,6 +1424,15 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
     wait_compute = std::max(wait_compute, dst->page_compute_seq[pg]);   // readers of the page's previous owner
     t.pt.push_back(pg);                                                 // (copies out of it are on this side stream)
   }
+  auto undo = [&]() {
+    for (auto it = t.pt.rbegin(); it != t.pt.rend(); ++it) dst->free_q.push_front(*it);
+    t = Session();
+    return TS_ERR_CUDA;
+  };
+#define TS_CUDA_UNDO(call)                    \
+  do {                                        \
+    if (!tc::cuda_ok((call), #call)) return undo(); \
+  } while (0)
   uint64_t seq_src = s.side_seq;
   if (n > 0) {
     int32_t* pairs = reinterpret_cast<int32_t*>(st->h);
@@ -1147,10 +1442,10 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
     }
     // (i) chunk boundary: after the compute work already enqueued on the session at the source, and after a resume
     // of it that may still be copying in
-    TS_CUDA(src->tl_compute.wait(dst->side, s.compute_seq));
-    TS_CUDA(src->tl_side.wait(dst->side, s.side_seq));
-    TS_CUDA(dst->tl_compute.wait(dst->side, wait_compute));
-    TS_CUDA(cudaMemcpyAsync(st->d, st->h, n * 8, cudaMemcpyHostToDevice, dst->side));
+    TS_CUDA_UNDO(src->tl_compute.wait(dst->side, s.compute_seq));
+    TS_CUDA_UNDO(src->tl_side.wait(dst->side, s.side_seq));
+    TS_CUDA_UNDO(dst->tl_compute.wait(dst->side, wait_compute));
+    TS_CUDA_UNDO(cudaMemcpyAsync(st->d, st->h, n * 8, cudaMemcpyHostToDevice, dst->side));
     PullParams p;
     p.src_slab = src->slab;
     p.dst_slab = dst->slab;
@@ -1158,16 +1453,18 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
     p.n_pages = (int32_t)n;
     p.vec_per_page = (int32_t)(dst->page_bytes / 16);
     p.page_stride = dst->page_bytes;
-    TS_CUDA(launch_page_pull(p, dst->sm_count, dst->side));   // (ii) the target fetches
+    TS_CUDA_UNDO(launch_page_pull(p, dst->sm_count, dst->side));   // (ii) the target fetches
+    // ---- the fetch is enqueued: from here on the move is carried through (the remaining calls only order streams)
     ++dst->launches;
-    TS_CUDA(cudaEventRecord(st->ev, dst->side));
+    cuda_ok(cudaEventRecord(st->ev, dst->side), "cudaEventRecord");
     st->in_flight = true;
     t.side_seq = dst->tl_side.record(dst->side);              // compute calls on the new session wait for this
     // (iii) the source's pages may be rewritten only after the fetch: mark that point on the source's side timeline
-    TS_CUDA(cudaSetDevice(a.device));
-    TS_CUDA(dst->tl_side.wait(src->side, t.side_seq));
+    cuda_ok(cudaSetDevice(a.device), "cudaSetDevice");
+    cuda_ok(dst->tl_side.wait(src->side, t.side_seq), "cudaStreamWaitEvent");
     seq_src = src->tl_side.record(src->side);
   }
+#undef TS_CUDA_UNDO
   t.ver = ++dst->ver_seq;
   t.state = TS_SESSION_RESIDENT;
   for (int32_t pg : s.pt) {                                   // release on the source (as a close would)
@@ -1196,12 +1493,17 @@ int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   if (rc != TS_OK) return rc;
   if (n == 0) return TS_OK;
   if (q_host == nullptr || k_host == nullptr || v_host == nullptr || out_host == nullptr) return TS_ERR_INVALID;
+  if (!(scale > 0.0f) || !std::isfinite(scale)) return TS_ERR_INVALID;
+  if ((flags & ~(uint32_t)TS_COMMIT) != 0) return TS_ERR_INVALID;
+  // all-or-nothing: the page demand of the step is checked before a single copy is enqueued
+  if (page_demand(pool, n, sids, chunk_frames) > (int64_t)pool->free_q.size()) return TS_ERR_NO_PAGES;
   const ts_pool_config& c = pool->cfg;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   TS_CUDA(cudaSetDevice(c.device));
   int64_t tokens = 0;
   for (int b = 0; b < n; ++b) tokens += (int64_t)chunk_frames[b] * c.frame_tokens;
-  const size_t tensor_bytes = align_up((size_t)tokens * c.n_heads * c.head_dim * 2, 1024);
+  const size_t nbytes = (size_t)tokens * c.n_heads * c.head_dim * 2;
+  const size_t tensor_bytes = align_up(nbytes, 1024);
   if (pool->h2d_s == nullptr) {
     TS_CUDA(cudaStreamCreateWithFlags(&pool->h2d_s, cudaStreamNonBlocking));
     TS_CUDA(cudaStreamCreateWithFlags(&pool->d2h_s, cudaStreamNonBlocking));
@@ -1209,14 +1511,14 @@ int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
       TS_CUDA(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
   }
   if (pool->stage_cap < 8 * tensor_bytes) {
-    if (pool->stage_dev) {
-      TS_CUDA(cudaDeviceSynchronize());
-      TS_CUDA(cudaFree(pool->stage_dev));
-      pool->stage_dev = nullptr;
-      pool->stage_cap = 0;
-    }
-    TS_CUDA(cudaMalloc((void**)&pool->stage_dev, 8 * tensor_bytes));
-    pool->stage_cap = 8 * tensor_bytes;
+    // Staging grows without waiting for anything: the outgrown buffer may still be read by launches in flight, so it is
+    // kept until the pool is destroyed (sizes double, so what is kept is less than what is in use).
+    uint8_t* fresh = nullptr;
+    const size_t cap = std::max(8 * tensor_bytes, 2 * pool->stage_cap);
+    TS_CUDA(cudaMalloc((void**)&fresh, cap));
+    if (pool->stage_dev) pool->retired.push_back(pool->stage_dev);
+    pool->stage_dev = fresh;
+    pool->stage_cap = cap;
     pool->host_steps = 0;
   }
   // Two staging sets and two copy streams: the H2D of this call does not wait for the caller's stream (host buffers
@@ -1229,21 +1531,27 @@ int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   uint8_t* dk = dq + tensor_bytes;
   uint8_t* dv = dk + tensor_bytes;
   uint8_t* dout = dv + tensor_bytes;
-  const size_t nbytes = (size_t)tokens * c.n_heads * c.head_dim * 2;
   if (slot_used) TS_CUDA(cudaStreamWaitEvent(pool->h2d_s, pool->ev_free[slot], 0));
-  TS_CUDA(cudaMemcpyAsync(dq, q_host, nbytes, cudaMemcpyHostToDevice, pool->h2d_s));
-  TS_CUDA(cudaMemcpyAsync(dk, k_host, nbytes, cudaMemcpyHostToDevice, pool->h2d_s));
-  TS_CUDA(cudaMemcpyAsync(dv, v_host, nbytes, cudaMemcpyHostToDevice, pool->h2d_s));
+  const uint8_t *hq = (const uint8_t*)q_host, *hk = (const uint8_t*)k_host, *hv = (const uint8_t*)v_host;
+  if (hk == hq + tensor_bytes && hv == hk + tensor_bytes) {   // one packed host buffer: one copy
+    TS_CUDA(cudaMemcpyAsync(dq, hq, 2 * tensor_bytes + nbytes, cudaMemcpyHostToDevice, pool->h2d_s));
+  } else {
+    TS_CUDA(cudaMemcpyAsync(dq, hq, nbytes, cudaMemcpyHostToDevice, pool->h2d_s));
+    TS_CUDA(cudaMemcpyAsync(dk, hk, nbytes, cudaMemcpyHostToDevice, pool->h2d_s));
+    TS_CUDA(cudaMemcpyAsync(dv, hv, nbytes, cudaMemcpyHostToDevice, pool->h2d_s));
+  }
   TS_CUDA(cudaEventRecord(pool->ev_in, pool->h2d_s));
   TS_CUDA(cudaStreamWaitEvent(stream, pool->ev_in, 0));
-  rc = ts_chunk_attention(pool, layer, n, sids, chunk_frames, dq, dk, dv, dout, nullptr, scale, cuda_stream);
-  if (rc != TS_OK) return rc;
+  // the product's best path: attention and append in ONE launch
+  rc = ts_chunk_step(pool, layer, n, sids, chunk_frames, dq, dk, dv, dout, nullptr, scale, flags, cuda_stream);
+  if (rc != TS_OK) {                                          // only a CUDA failure can get here (everything else was checked)
+    cudaEventRecord(pool->ev_free[slot], stream);             // the set's next user still waits for what was enqueued
+    return rc;
+  }
   TS_CUDA(cudaEventRecord(pool->ev_attn, stream));
   TS_CUDA(cudaStreamWaitEvent(pool->d2h_s, pool->ev_attn, 0));
   TS_CUDA(cudaMemcpyAsync(out_host, dout, nbytes, cudaMemcpyDeviceToHost, pool->d2h_s));
   TS_CUDA(cudaEventRecord(pool->ev_out, pool->d2h_s));
-  rc = ts_kv_append(pool, layer, n, sids, chunk_frames, dk, dv, flags, cuda_stream);
-  if (rc != TS_OK) return rc;
   TS_CUDA(cudaStreamWaitEvent(stream, pool->ev_out, 0));   // stream order: out_host is complete when the call is
   TS_CUDA(cudaEventRecord(pool->ev_free[slot], stream));   // ... and the staging set is free again
   return TS_OK;

@@ -567,6 +567,63 @@ def test_chunk_step_host_two_steps():
         assert np.abs(o_gpu - o_ref).max() <= 2e-2
         assert rel_l2(o_gpu, o_ref) <= 5e-3
     dp.check_state(sids, kv=True)
+    # a packed host buffer [3][tokens][H][D] (one H2D) and a larger batch than before (the staging grows, no device sync)
+    cf = [3, 3]
+    n_tok = sum(cf) * T
+    q, k, v = (draw(rng, n_tok, shape) for _ in range(3))
+    o_ref, _ = oracle.chunk_attention(dp.o, 0, sids, cf, q, k, v, scale_of(shape))
+    packed = torch.from_numpy(np.stack([q, k, v]).view(np.int16)).pin_memory()
+    assert packed[0].numel() * 2 % 1024 == 0                   # tensors sit 1024-byte aligned behind each other
+    hout = torch.zeros_like(packed[0]).pin_memory()
+    dp.g.ts_chunk_step_host(0, sids, cf, packed[0], packed[1], packed[2], hout, float(scale_of(shape)), TS_COMMIT)
+    dp.o.append(0, sids, cf, k, v, commit=True)
+    torch.cuda.synchronize()
+    o_gpu = hout.view(torch.bfloat16).double().numpy()
+    assert np.abs(o_gpu - o_ref).max() <= 2e-2 and rel_l2(o_gpu, o_ref) <= 5e-3
+    dp.check_state(sids, kv=True)
+    dp.g.close()
+
+
+def test_chunk_step_host_is_all_or_nothing():
+    """TS_ERR_NO_PAGES from the host-buffer step: nothing was enqueued (out_host keeps its sentinel, no kernel was
+    launched), no table or free-list entry changed, and the next valid call runs as if the failed one had not happened."""
+    import paper_2606_19271_b200 as tc
+    shape = shape_of(n_heads=2, head_dim=128, frame_tokens=100, window_frames=0, page_tokens=64, n_pages=7)
+    rng = np.random.default_rng(12)
+    dp = DualPool(shape, None)
+    T = shape.frame_tokens
+    a, b = dp.open(), dp.open()
+    scale = float(scale_of(shape))
+
+    def host(bits):
+        return torch.from_numpy(bits.view(np.int16)).pin_memory()
+
+    q, k, v = (draw(rng, 2 * T, shape) for _ in range(3))       # a: 1 frame, b: 1 frame -> 2 + 2 pages: fits
+    o_ref, _ = oracle.chunk_attention(dp.o, 0, [a, b], [1, 1], q, k, v, scale_of(shape))
+    h1 = [host(x) for x in (q, k, v)] + [torch.zeros(2 * T, 2, 128, dtype=torch.int16).pin_memory()]
+    dp.g.ts_chunk_step_host(0, [a, b], [1, 1], *h1, scale, tc.TS_COMMIT)
+    dp.o.append(0, [a, b], [1, 1], k, v, commit=True)
+    torch.cuda.synchronize()
+    launches = dp.g.ts_pool_launch_count()
+    q2, k2, v2 = (draw(rng, 4 * T, shape) for _ in range(3))    # 2 + 2 more frames: 300 tokens each = 5 pages each > 7
+    sentinel = torch.full((4 * T, 2, 128), 0x1234, dtype=torch.int16).pin_memory()
+    h2 = [host(x) for x in (q2, k2, v2)]
+    with pytest.raises(tc.TurboChunkError) as e:
+        dp.g.ts_chunk_step_host(0, [a, b], [2, 2], *h2, sentinel, scale, tc.TS_COMMIT)
+    assert e.value.code == tc.TS_ERR_NO_PAGES
+    torch.cuda.synchronize()
+    assert dp.g.ts_pool_launch_count() == launches and bool((sentinel == 0x1234).all())
+    dp.check_state([a, b])
+    q3, k3, v3 = (draw(rng, 2 * T, shape) for _ in range(3))    # one more frame for a only: fits
+    o3, _ = oracle.chunk_attention(dp.o, 0, [a], [2], q3, k3, v3, scale_of(shape))
+    h3 = [host(x) for x in (q3, k3, v3)] + [torch.zeros(2 * T, 2, 128, dtype=torch.int16).pin_memory()]
+    dp.g.ts_chunk_step_host(0, [a], [2], *h3, scale, tc.TS_COMMIT)
+    dp.o.append(0, [a], [2], k3, v3, commit=True)
+    torch.cuda.synchronize()
+    for hout, ref in ((h1[3], o_ref), (h3[3], o3)):
+        o_gpu = hout.view(torch.bfloat16).double().numpy()
+        assert np.abs(o_gpu - ref).max() <= 2e-2 and rel_l2(o_gpu, ref) <= 5e-3
+    dp.check_state([a, b])
     dp.g.close()
 
 
