@@ -1,20 +1,25 @@
 #!/usr/bin/env python
 """bench.py — coalesced chunk step on BASELINE.json configs[2] (Wan-1.3B-shaped 8-session batch).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras]
 
 One JSON line on stdout (rank 0).  A "step" is one pass of the hot path over one coalesced batch:
     resume(idle session X) on the side stream                      (a6)
     open + close of a transient session                            (a7)
+    every COMMIT_EVERY-th step: the transient session's first chunk as a real committed step - page growth, a
+        schedule build for it AND (single-entry schedule cache) a rebuild for the main batch, commit (a1, a3, a4)
     ts_chunk_step(batch of 8, flags=0)    scheduler + attention (a1, a2) and paged scatter (a3) in ONE launch: the
                                           scatter is done by the two role-less warps of every attention CTA
     suspend(X) on the side stream                                  (a5)
-flags=0 keeps every timed step on the identical drawn state of configs[2]; the window roll (a4) is host
-integer arithmetic inside ts_kv_append(TS_COMMIT), exercised by the tests, not by the timed loop.
-`value` = attention FLOPs of the batch / step time (all ranks); `roofline` (attention) and `append` are the two
-kernels timed alone with CUDA events, one after the other, in a second loop over the same steps;
-`e2e` is the same step through ts_chunk_step_host with pinned HOST buffers (H2D of Q/K/V and D2H of O inside
-the timed region).  N > 1 runs N independent replicas (sessions are independent units).
+flags=0 on the main batch keeps every timed step on the identical drawn state of configs[2].
+`value` = attention FLOPs of all launches / time of the K steps (all ranks).  `roofline` comes from the SAME loop:
+CUDA events around every fused launch of the main batch on the launching stream (so ms_per_launch <= ms_per_step),
+with the SM clock measured inside the kernel (clock64 / globaltimer, ts_pool_clock_probe).  `sustained` repeats
+the step back to back for >= 2 s.  `kernels_alone` times attention and append as separate launches (the append's
+roofline).  `e2e` is the same step through ts_chunk_step_host with pinned HOST buffers (H2D of Q/K/V and D2H of O
+inside the timed region).  `configs` carries configs[1], [3] (one layer, and the 40-layer step eager and as one CUDA
+graph) and [4] (200-step churn); `overlap` the cost of a full-window offload under the step (NEXT-1); `latency_model`
+the measured l_hat(n).  N > 1 runs N independent replicas (sessions are independent units).
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
 """
 import argparse
@@ -35,9 +40,10 @@ UNIT = "TFLOP/s"
 WORKLOAD = "configs[2] wan13b_batch: 8 sessions x 12 heads x D128, T=1560, 3-frame chunks, W=21, B=256"
 NOMINAL_BF16_TFLOPS = 2250.0
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+COMMIT_EVERY = 4
 # dram__bytes_read.sum + dram__bytes_write.sum of one attention launch on this workload, from the ncu --set full
-# capture summarised in profiles/ (None until a capture exists).
-ATTENTION_DRAM_TRAFFIC_BYTES = 1037573888  # 934.57 MB read + 103.00 MB write (attention-only launch), profiles/r1_final_build.txt
+# capture summarised in the file named beside it (not a measurement of this run).
+ATTENTION_DRAM_TRAFFIC = {"bytes": 1037573888, "from": "profiles/r1_final_build.txt (ncu --set full, attention-only launch)"}
 
 
 def load_peaks():
@@ -48,11 +54,21 @@ def load_peaks():
     return dict(FALLBACK_PEAKS), "fallback"
 
 
-class ClockSampler:
-    """Samples SM clock and throttle reasons while the timed region runs (B200_PROFILING.md clocks line)."""
+def config_dict(w, world):
+    """The workload description both arms print (the driver compares them key by key)."""
+    import synth
+    return {"workload": WORKLOAD, "prior_frames": [s.prior_frames for s in w.sessions],
+            "attention_tflop_per_step": round(synth.attention_flops(w.shape, w.sessions) / 1e12, 4),
+            "l2": "inputs larger than L2 (Q/K/V 345 MB + KV cache 1.1 GB per step vs 126 MB L2)",
+            "parallelism": f"replicas x{world} (sessions are independent; no collective)"}
 
-    def __init__(self, index):
-        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons while the timed region runs (B200_PROFILING.md clocks line).  NVML reports
+    the clock BETWEEN launches of a few ms; the clock under the kernel is measured in the kernel (clock probe)."""
+
+    def __init__(self, index, period=0.005):
+        self.index, self.samples, self.reasons, self.max_mhz, self.period = index, [], set(), None, period
         self._stop = threading.Event()
         self._thread = None
         try:
@@ -84,7 +100,7 @@ class ClockSampler:
                         self.reasons.add(name)
             except Exception:
                 pass
-            self._stop.wait(0.02)
+            self._stop.wait(self.period)
 
     def __enter__(self):
         if self.nv is not None:
@@ -100,7 +116,31 @@ class ClockSampler:
     def summary(self):
         if not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
-        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_min_mhz": float(np.min(self.samples)),
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "nvml_samples": len(self.samples)}
+
+
+class KernelClock:
+    """SM clock under the attention kernel itself: CTA 0 accumulates clock64 cycles and globaltimer nanoseconds."""
+
+    def __init__(self, pool, device):
+        import torch
+        self.pool = pool
+        self.buf = torch.zeros(2, dtype=torch.int64, device=device)
+
+    def __enter__(self):
+        self.buf.zero_()
+        self.pool.ts_pool_clock_probe(self.buf)
+        return self
+
+    def __exit__(self, *exc):
+        self.pool.ts_pool_clock_probe(None)
+
+    def mhz(self):
+        import torch
+        torch.cuda.synchronize()
+        cyc, ns = (int(x) for x in self.buf.tolist())
+        return round(cyc / ns * 1e3, 1) if ns > 0 else None
 
 
 def dist_env():
@@ -168,31 +208,44 @@ def build_workload(device, with_oracle):
     pool.ts_kv_append(0, [x], [idle_frames], xk, xk, TS_COMMIT)
     pool.ts_session_suspend(x)
     pool.ts_offload_sync()
+    # the transient session's first chunk (1 frame): q = k = v of the first T tokens
+    tq = q[:T].contiguous()
     torch.cuda.synchronize(device)
     return {"w": w, "pool": pool, "opool": opool, "sids": sids, "cf": [3] * len(sids), "q": q, "k": k, "v": v,
-            "x": x, "x_pages": pool.ts_session_info(x)["n_pages"], "chunks": chunks, "to_bits": to_bits}
+            "x": x, "x_pages": pool.ts_session_info(x)["n_pages"], "chunks": chunks, "to_bits": to_bits,
+            "tq": tq, "tout": torch.empty_like(tq),
+            "t_flops": 4 * D * H * synth.attention_pairs(0, 1, T, sh.window_frames)}
 
 
-def step_device(wl, out):
-    """One coalesced chunk step, inputs resident in HBM."""
+def step_device(wl, out, i=0, ev=None):
+    """One coalesced chunk step, inputs resident in HBM.  Returns the attention FLOPs it launched."""
+    from paper_2606_19271_b200 import TS_COMMIT
     pool = wl["pool"]
+    scale = float(wl["w"].scale)
+    flops = wl["flops_step"]
     pool.ts_session_resume(wl["x"])
     t = pool.ts_session_open()
+    if i % COMMIT_EVERY == COMMIT_EVERY - 1:
+        pool.ts_chunk_step(0, [t], [1], wl["tq"], wl["tq"], wl["tq"], wl["tout"], None, scale, TS_COMMIT)
+        flops += wl["t_flops"]
     pool.ts_session_close(t)
-    pool.ts_chunk_step(0, wl["sids"], wl["cf"], wl["q"], wl["k"], wl["v"], out, None, float(wl["w"].scale), 0)
+    if ev is not None:
+        ev[0].record()
+    pool.ts_chunk_step(0, wl["sids"], wl["cf"], wl["q"], wl["k"], wl["v"], out, None, scale, 0)
+    if ev is not None:
+        ev[1].record()
     pool.ts_session_suspend(wl["x"])
+    return flops
 
 
 def step_kernels(wl, out, ev):
-    """The same step with attention and append as separate calls on one stream, for per-kernel timing."""
+    """The same batch with attention and append as separate launches on one stream, for per-kernel timing."""
     pool = wl["pool"]
-    pool.ts_session_resume(wl["x"])
     ev[0].record()
     pool.ts_chunk_attention(0, wl["sids"], wl["cf"], wl["q"], wl["k"], wl["v"], out, None, float(wl["w"].scale))
     ev[1].record()
     pool.ts_kv_append(0, wl["sids"], wl["cf"], wl["k"], wl["v"], 0)
     ev[2].record()
-    pool.ts_session_suspend(wl["x"])
 
 
 def step_host(wl, hq, hk, hv, hout):
@@ -248,9 +301,9 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extras", action="store_true",
+                    help="only the timed loop, the roofline and e2e (skips sustained / configs / overlap / latency_model)")
     args = ap.parse_args()
-    if args.warmup < 3:
-        args.warmup = 3
     rank, world, local = dist_env()
 
     import torch
@@ -260,9 +313,11 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return 0
-        run_reference(args)
+        run_reference(args, world)
         return 0
 
+    if args.warmup < 3:
+        args.warmup = 3                     # timing rule: at least 3 warm-up steps on the GPU
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     device = torch.device("cuda", local)
@@ -271,63 +326,80 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=device)
     peaks, peaks_kind = load_peaks()
+    extras = (world == 1) and not args.no_extras
 
     wl = build_workload(device, with_oracle=(rank == 0 and world == 1))
     pool, w = wl["pool"], wl["w"]
     sh = w.shape
     flops_step = synth.attention_flops(sh, w.sessions)
+    wl["flops_step"] = flops_step
     tokens = wl["q"].shape[0]
     append_bytes = 4 * tokens * sh.n_heads * sh.head_dim * 2            # read K,V + write K,V
     out = torch.empty_like(wl["q"])
+    kclock = KernelClock(pool, device)
 
     def barrier():
         if world > 1:
             torch.distributed.barrier()
         torch.cuda.synchronize(device)
 
-    # ---- device-resident timing
-    for _ in range(args.warmup):
-        step_device(wl, out)
+    # ---- device-resident timing: `value` and the attention roofline come from this one loop
+    for i in range(args.warmup):
+        step_device(wl, out, i)
         join_side(pool)
     barrier()
     t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     step_evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
-    launches0 = pool.ts_pool_launch_count()
-    with ClockSampler(device.index if device.index is not None else 0) as clocks:
+    launch_evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
+    launches0, builds0 = pool.ts_pool_launch_count(), pool.ts_pool_sched_builds()
+    flops_loop, host_s = 0.0, 0.0
+    with ClockSampler(device.index if device.index is not None else 0) as clocks, kclock:
         t_begin.record()
         for i in range(args.steps):
             step_evs[i][0].record()
-            step_device(wl, out)
+            h0 = time.perf_counter()
+            flops_loop += step_device(wl, out, i, launch_evs[i])
+            host_s += time.perf_counter() - h0
             join_side(pool)
             step_evs[i][1].record()
         t_end.record()
         barrier()
+        clock_in_kernel = kclock.mhz()
     launches = pool.ts_pool_launch_count() - launches0
+    builds = pool.ts_pool_sched_builds() - builds0
+    # host cost of a step's calls with an empty queue behind them (in the loop above the host runs ahead of the GPU until
+    # the 8-deep staging ring pushes back, so its wall time there is mostly waiting)
+    host_unblocked = []
+    for i in range(2 * COMMIT_EVERY):
+        torch.cuda.synchronize(device)
+        h0 = time.perf_counter()
+        step_device(wl, out, i)
+        host_unblocked.append((time.perf_counter() - h0) * 1e3)
+        join_side(pool)
+    torch.cuda.synchronize(device)
     ms_total = t_begin.elapsed_time(t_end)
     step_ms_max = float(max(e[0].elapsed_time(e[1]) for e in step_evs))
+    attn_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in launch_evs]))
 
-    # ---- the two kernels alone (same steps, attention and append as separate calls on one stream).  The GPU is
-    # power-capped: a short idle gap lets this loop start from the same power state as the timed loop above.
+    backend_dev = device
+    ms_total_all, flops_all = aggregate(ms_total, flops_loop, world, backend_dev)
+
+    # ---- the two kernels as separate launches (the append's roofline).  The GPU is power-capped: a short idle gap
+    # lets this loop start from the same power state as the timed loop above.
     time.sleep(0.5)
     for _ in range(args.warmup):
         step_kernels(wl, out, [torch.cuda.Event(enable_timing=True) for _ in range(3)])
-        join_side(pool)
     barrier()
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
     for i in range(args.steps):
         step_kernels(wl, out, evs[i])
-        join_side(pool)
     barrier()
-    attn_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    attn_alone_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
     append_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
 
-    # ---- offload leg (side stream, timed alone): suspend / resume of a full-window session
-    off = measure_offload(wl)
-    off["scattered"] = {k: v for k, v in measure_offload(wl, permuted=True).items() if k in ("d2h", "h2d", "placement")}
-    mig = measure_migration(wl, peaks["hbm_gbs"])
-
-    # ---- end to end through ts_chunk_step_host with pinned host buffers
-    hq, hk, hv = (t.cpu().pin_memory() for t in (wl["q"], wl["k"], wl["v"]))
+    # ---- end to end through ts_chunk_step_host with pinned host buffers (one packed [3][tokens][H][D] input buffer)
+    hin = torch.stack([t.cpu() for t in (wl["q"], wl["k"], wl["v"])]).pin_memory()
+    hq, hk, hv = hin[0], hin[1], hin[2]
     hout = torch.empty_like(hq).pin_memory()
     for _ in range(3):
         step_host(wl, hq, hk, hv, hout)
@@ -343,51 +415,486 @@ def main():
     e2e_ms = e0.elapsed_time(e1)
     h2d = 3 * hq.numel() * 2 + wl["x_pages"] * pool.page_bytes
     d2h = hq.numel() * 2 + wl["x_pages"] * pool.page_bytes
-
-    backend_dev = device
-    ms_total_all, flops_all = aggregate(ms_total, flops_step * args.steps, world, backend_dev)
     e2e_ms_all, _ = aggregate(e2e_ms, 0.0, world, backend_dev)
+    link = measure_link(device, h2d, d2h) if rank == 0 else None
+
     if rank != 0:
+        if world > 1:
+            torch.distributed.barrier()       # rank 0's migrate_p2p leg runs while the others wait here
         return 0
 
     value = flops_all / (ms_total_all * 1e-3) / 1e12
     achieved = flops_step / (attn_ms * 1e-3) / 1e12
     peak = peaks["bf16_tflops"]
+    sust_peak = peaks.get("bf16_tflops_sustained", peak)
+    clk = clocks.summary()
+    clk["sm_mhz_in_kernel"] = clock_in_kernel
+    clk["note"] = "sm_mhz: NVML between launches; sm_mhz_in_kernel: clock64/globaltimer inside the attention kernel"
     result = {
         "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": round(ms_total_all / args.steps, 4), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "prior_frames": [s.prior_frames for s in w.sessions],
-                   "attention_tflop_per_step": round(flops_step / 1e12, 4), "append_flags": 0,
-                   "l2": "inputs larger than L2 (Q/K/V 345 MB + KV cache 1.1 GB per step vs 126 MB L2)",
-                   "parallelism": f"replicas x{world} (sessions are independent; no collective)"},
+        "config": config_dict(w, world),
+        "step": {"append_flags_main_batch": 0, "commit_every": COMMIT_EVERY,
+                 "committed_step": "transient session, 1 frame, P=0: page growth + schedule build + commit; evicts the "
+                                   "single-entry schedule cache, so the main batch's schedule is rebuilt too",
+                 "sched_builds_in_timed_loop": int(builds), "host_ms_per_step_in_loop": round(host_s / args.steps * 1e3, 4),
+                 "host_ms_per_step_unblocked": {"cached_schedule": round(float(np.min(host_unblocked)), 4),
+                                                "with_committed_step_and_rebuild": round(float(np.max(host_unblocked)), 4)}},
         "max_chunk_latency_ms": round(step_ms_max, 4),
-        "roofline": {"bound": "tensor", "kernel": "chunk_attention_kernel<128>", "achieved": round(achieved, 2),
-                     "peak": peak, "unit": "TFLOP/s", "frac": round(achieved / peak, 4),
+        "roofline": {"bound": "tensor", "kernel": "chunk_attention_kernel<128> (fused: + the batch's KV append)",
+                     "achieved": round(achieved, 2), "peak": peak, "unit": "TFLOP/s", "frac": round(achieved / peak, 4),
                      "peak_kind": f"{peaks_kind} burst cuBLAS bf16 (MEASURED_PEAKS.json)",
-                     "frac_of_sustained": round(achieved / peaks.get("bf16_tflops_sustained", peak), 4),
+                     "frac_of_sustained": round(achieved / sust_peak, 4),
                      "frac_of_nominal_2250": round(achieved / NOMINAL_BF16_TFLOPS, 4),
-                     "ms_per_launch": round(attn_ms, 4), "traffic": ATTENTION_DRAM_TRAFFIC_BYTES},
+                     "ms_per_launch": round(attn_ms, 4), "timed_in": "the loop `value` comes from (events around each launch)",
+                     "sm_mhz_in_kernel": clock_in_kernel,
+                     "traffic": ATTENTION_DRAM_TRAFFIC["bytes"], "traffic_from": ATTENTION_DRAM_TRAFFIC["from"]},
+        "kernels_alone": {"note": "separate launches, second loop after a 0.5 s idle gap (another power state)",
+                          "attention_ms": round(attn_alone_ms, 4),
+                          "attention_tflops": round(flops_step / (attn_alone_ms * 1e-3) / 1e12, 2)},
         "append": {"bound": "hbm", "kernel": "kv_append_kernel", "bytes_per_launch": append_bytes,
                    "ms_per_launch": round(append_ms, 4), "achieved": round(append_bytes / (append_ms * 1e-3) / 1e9, 1),
                    "peak": peaks["hbm_gbs"], "unit": "GB/s",
                    "frac": round(append_bytes / (append_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], 4)},
-        "offload": off,
-        "migrate": mig,
         "e2e": {"value": round(flops_step * args.steps * world / (e2e_ms_all * 1e-3) / 1e12, 2), "unit": UNIT,
                 "ms_per_step": round(e2e_ms_all / args.steps, 4), "h2d_bytes_per_step": int(h2d),
-                "d2h_bytes_per_step": int(d2h), "api": "ts_chunk_step_host (pinned host Q/K/V/O)"},
+                "d2h_bytes_per_step": int(d2h),
+                "api": "ts_chunk_step_host (pinned host Q/K/V packed in one buffer, O; one fused launch per step)",
+                "link": e2e_link(link, h2d, d2h, e2e_ms_all / args.steps)},
         "gpu_launches": int(launches),
-        "clocks": clocks.summary(),
+        "clocks": clk,
     }
+    # ---- legs that do not feed `value` (single GPU only)
+    result["offload"] = measure_offload(wl)
+    result["offload"]["scattered"] = {k: v for k, v in measure_offload(wl, permuted=True).items()
+                                      if k in ("d2h", "h2d", "placement")}
+    result["migrate"] = measure_migration(wl, peaks["hbm_gbs"])
+    if world > 1 and torch.cuda.device_count() >= 2:
+        result["migrate_p2p"] = measure_migration_p2p(wl)
+    if extras:
+        result["sustained"] = measure_sustained(wl, out, kclock, device, sust_peak, peak)
+        result["overlap"] = measure_overlap(wl, out)
+        pool.close()
+        wl["pool"] = None
+        torch.cuda.empty_cache()
+        result["latency_model"] = measure_latency_model()
+        result["configs"] = {"configs[1]": run_config1(device, peak), "configs[3]": run_config3(device, peak),
+                             "configs[4]": run_config4(device, peak)}
     if world == 1:
         chunk_bits = [tuple(wl["to_bits"](t) for t in c) for c in wl["chunks"]]
         dt, fl, desc = oracle_sample(w, wl["opool"], wl["sids"], chunk_bits)
         result["cpu_baseline"] = {"value": round(fl / dt / 1e12, 5), "unit": UNIT, "cores": cpu_threads(),
                                   "kind": "oracle", "sample": desc, "seconds": round(dt, 2)}
     print(json.dumps(result))
-    pool.close()
+    if wl["pool"] is not None:
+        wl["pool"].close()
+    if world > 1:
+        torch.distributed.barrier()
     return 0
+
+
+# ------------------------------------------------------------------------------------------------ legs
+def measure_link(device, h2d_bytes, d2h_bytes):
+    """The host link of this box, this run: one pinned copy each way alone, and both at once with the step's byte mix."""
+    import torch
+    n_in, n_out = int(h2d_bytes), int(d2h_bytes)
+    hin = torch.empty(n_in, dtype=torch.uint8).pin_memory()
+    hout = torch.empty(n_out, dtype=torch.uint8).pin_memory()
+    din = torch.empty(n_in, dtype=torch.uint8, device=device)
+    dout = torch.empty(n_out, dtype=torch.uint8, device=device)
+    s_in, s_out = torch.cuda.Stream(device), torch.cuda.Stream(device)
+    res = {}
+
+    def run(do_in, do_out):
+        best = 1e9
+        for _ in range(5):
+            torch.cuda.synchronize(device)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            s_in.wait_event(a)
+            s_out.wait_event(a)
+            if do_in:
+                with torch.cuda.stream(s_in):
+                    din.copy_(hin, non_blocking=True)
+            if do_out:
+                with torch.cuda.stream(s_out):
+                    hout.copy_(dout, non_blocking=True)
+            torch.cuda.current_stream().wait_stream(s_in)
+            torch.cuda.current_stream().wait_stream(s_out)
+            b.record()
+            torch.cuda.synchronize(device)
+            best = min(best, a.elapsed_time(b))
+        return best
+    res["h2d_alone_gbs"] = n_in / (run(True, False) * 1e-3) / 1e9
+    res["d2h_alone_gbs"] = n_out / (run(False, True) * 1e-3) / 1e9
+    res["both_ms"] = run(True, True)
+    return res
+
+
+def e2e_link(link, h2d, d2h, ms_per_step):
+    if link is None:
+        return None
+    return {"h2d_gbs_in_step": round(h2d / (ms_per_step * 1e-3) / 1e9, 2),
+            "h2d_alone_gbs": round(link["h2d_alone_gbs"], 2), "d2h_alone_gbs": round(link["d2h_alone_gbs"], 2),
+            "frac_of_h2d_alone": round(h2d / (ms_per_step * 1e-3) / 1e9 / link["h2d_alone_gbs"], 4),
+            "both_directions_ms": round(link["both_ms"], 4),
+            "frac_of_both_directions": round(link["both_ms"] / ms_per_step, 4),
+            "note": "the step moves h2d and d2h bytes at once; `both_directions_ms` is the same byte mix as two plain "
+                    "pinned copies running concurrently (the link's own limit for this step), best of 5, same run"}
+
+
+def measure_sustained(wl, out, kclock, device, sust_peak, burst_peak, seconds=2.0):
+    """The step back to back for >= `seconds`: the power-capped regime."""
+    import torch
+    pool = wl["pool"]
+    time.sleep(0.5)
+    for i in range(3):
+        step_device(wl, out, i)
+        join_side(pool)
+    torch.cuda.synchronize(device)
+    n_guess = max(50, int(seconds * 1e3 / 2.4))
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    flops, steps, ms = 0.0, 0, 0.0
+    with ClockSampler(device.index if device.index is not None else 0, period=0.02) as clocks, kclock:
+        while ms < seconds * 1e3:
+            a.record()
+            for i in range(n_guess):
+                flops += step_device(wl, out, steps + i)
+                join_side(pool)
+            b.record()
+            torch.cuda.synchronize(device)
+            ms += a.elapsed_time(b)
+            steps += n_guess
+            n_guess = 100
+        mhz = kclock.mhz()
+    tfl = flops / (ms * 1e-3) / 1e12
+    c = clocks.summary()
+    return {"seconds": round(ms / 1e3, 3), "steps": steps, "value": round(tfl, 2), "unit": UNIT,
+            "ms_per_step": round(ms / steps, 4), "peak": sust_peak,
+            "frac": round(tfl / sust_peak, 4), "frac_of_burst": round(tfl / burst_peak, 4),
+            "frac_of_nominal_2250": round(tfl / NOMINAL_BF16_TFLOPS, 4), "sm_mhz_in_kernel": mhz,
+            "nvml": {"sm_mhz_median": c.get("sm_mhz"), "sm_mhz_min": c.get("sm_min_mhz"), "reasons": c.get("reasons")},
+            "peak_kind": "bf16_tflops_sustained (MEASURED_PEAKS.json): cuBLAS back to back for 4 s"}
+
+
+def measure_overlap(wl, out, reps=12):
+    """SURVEY.md §8(f) NEXT-1 (PAPER.md:76 (iii), :160): the configs[2] step alone, and the same step while a FULL-window
+    (21-frame, 201 MB) idle session is resumed and another suspended on the side stream.  Step time by events on the
+    compute stream, offload rate by events on the side stream; `resume_done_before_step_end` says whether a session
+    resumed at the start of step t is ready when step t ends (it is served in step t+1 without a wait)."""
+    import torch
+    from synth.draw import draw_bits_torch
+    from paper_2606_19271_b200 import TS_COMMIT, TurboChunkPool
+    w = wl["w"]
+    sh = w.shape
+    T, H, D = sh.frame_tokens, sh.n_heads, sh.head_dim
+    dev = wl["q"].device
+    # a second pool for the two idle full-window sessions would not share the step's free list; use the main pool's twin:
+    # same geometry, the batch of configs[2] re-created in it plus two full-window idle sessions Y, Z
+    n_pages = sh.n_pages + 2 * 130
+    pool = TurboChunkPool(1, H, D, sh.page_tokens, n_pages, T, sh.window_frames, sh.max_sessions,
+                          free_order=np.random.default_rng(5).permutation(n_pages), host_pages=2 * 130, device=dev.index)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(w.seed)
+    sids = []
+    for spec in w.sessions:
+        sid = pool.ts_session_open()
+        for _ in range(0, spec.prior_frames, 3):
+            dk = draw_bits_torch(gen, 3 * T, H, D, dev)
+            pool.ts_kv_append(0, [sid], [3], dk, dk, TS_COMMIT)
+        sids.append(sid)
+    idle = []
+    for _ in range(2):
+        s = pool.ts_session_open()
+        for _ in range(7):
+            dk = draw_bits_torch(gen, 3 * T, H, D, dev)
+            pool.ts_kv_append(0, [s], [3], dk, dk, TS_COMMIT)
+        idle.append(s)
+    y, z = idle
+    pool.ts_session_suspend(y)
+    pool.ts_offload_sync()
+    nbytes = pool.ts_session_info(y)["n_pages"] * pool.page_bytes
+    side = pool.side_stream
+    scale = float(w.scale)
+    cur = torch.cuda.current_stream()
+
+    def step():
+        pool.ts_chunk_step(0, sids, wl["cf"], wl["q"], wl["k"], wl["v"], out, None, scale, 0)
+
+    for _ in range(3):
+        step()
+    torch.cuda.synchronize()
+    # steady state: `n_steps` steps back to back (the host runs ahead, as in serving), alone and under continuous offload
+    n_steps, alone, loaded, h2d_ms, d2h_ms = 8, [], [], [], []
+    for r in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(n_steps):
+            step()
+        b.record()
+        torch.cuda.synchronize()
+        alone.append(a.elapsed_time(b) / n_steps)
+    for r in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(7)]
+        a.record()
+        side.wait_event(a)                     # the offload starts with the first step
+        evs[0].record(side)
+        for i in range(3):                     # 3 x (resume 201 MB H2D, suspend 201 MB D2H): ~25 ms of side-stream work
+            pool.ts_session_resume(y)
+            evs[2 * i + 1].record(side)
+            pool.ts_session_suspend(z)
+            evs[2 * i + 2].record(side)
+            y, z = z, y
+        for _ in range(n_steps):
+            step()
+        b.record()
+        torch.cuda.synchronize()
+        loaded.append(a.elapsed_time(b) / n_steps)
+        h2d_ms += [evs[2 * i].elapsed_time(evs[2 * i + 1]) for i in range(3)]
+        d2h_ms += [evs[2 * i + 1].elapsed_time(evs[2 * i + 2]) for i in range(3)]
+    pool.close()
+    alone_ms, loaded_ms = float(np.median(alone)), float(np.median(loaded))
+    h2d, d2h = float(np.median(h2d_ms)), float(np.median(d2h_ms))
+    return {"steps_back_to_back": n_steps, "step_alone_ms": round(alone_ms, 4), "step_with_offload_ms": round(loaded_ms, 4),
+            "step_slowdown": round(loaded_ms / alone_ms - 1.0, 4), "offload_bytes_each_way": int(nbytes),
+            "resume_h2d_gbs_under_load": round(nbytes / (h2d * 1e-3) / 1e9, 2),
+            "suspend_d2h_gbs_under_load": round(nbytes / (d2h * 1e-3) / 1e9, 2),
+            "resume_ms": round(h2d, 4), "steps_to_hide_one_resume": round(h2d / loaded_ms, 2),
+            "resume_done_within_steps": int(np.ceil(h2d / loaded_ms)),
+            "note": "a full-window (201 MB) resume takes `resume_ms` at the link rate, i.e. `steps_to_hide_one_resume` steps of "
+                    "this batch: a session whose resume is enqueued at the start of step t is served in step "
+                    "t + resume_done_within_steps without any host wait (the step's launch waits on the resume's event), "
+                    "and the steps it hides behind run `step_slowdown` slower"}
+
+
+def measure_latency_model(ns=(1, 2, 4, 5, 6, 8, 16, 32), layers=30, passes=4, slo_ms=670.0):
+    """l_hat(n): per-layer attention + append time against the number of co-located full-window sessions,
+    and the largest n whose 30-layer x 4-pass lower bound meets the 670 ms SLO."""
+    from paper_2606_19271_b200.latency_model import measure
+    rows, best = [], 0
+    for n in ns:
+        attn_ms, app_ms, tfl = measure(n, 18, 12, 128, 1560, 21, 256, reps=5)
+        step_ms = layers * (passes * attn_ms + app_ms)
+        if step_ms <= slo_ms:
+            best = max(best, n)
+        rows.append({"n": n, "attention_ms_per_layer": round(attn_ms, 4), "append_ms_per_layer": round(app_ms, 4),
+                     "attention_tflops": round(tfl, 1), "chunk_step_ms_lower_bound": round(step_ms, 1)})
+    per = [r["attention_ms_per_layer"] / r["n"] for r in rows]
+    return {"shape": "Wan-1.3B attention, every session at the full 21-frame window, one layer", "l_hat": rows,
+            "ms_per_session_layer_min_max": [round(min(per), 4), round(max(per), 4)],
+            "model": f"{layers} layers x ({passes} passes attention + 1 append); projections/MLP are outside this library",
+            "slo_ms": slo_ms, "largest_n_under_slo": best}
+
+
+def _timed(fn, reps, device):
+    import torch
+    ts = []
+    for _ in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        torch.cuda.synchronize(device)
+        ts.append(a.elapsed_time(b))
+    return ts
+
+
+def run_config1(device, peak):
+    """configs[1]: one session, 12 heads, P = 6, c = 3."""
+    import torch
+    import synth
+    from synth.draw import draw_bits_torch
+    from paper_2606_19271_b200 import TS_COMMIT, TurboChunkPool
+    w = synth.wan13b_single()
+    sh = w.shape
+    T, H, D = sh.frame_tokens, sh.n_heads, sh.head_dim
+    pool = TurboChunkPool(1, H, D, sh.page_tokens, sh.n_pages, T, sh.window_frames, sh.max_sessions, device=device.index)
+    gen = torch.Generator(device=device)
+    gen.manual_seed(w.seed)
+    sid = pool.ts_session_open()
+    for _ in range(2):
+        dk = draw_bits_torch(gen, 3 * T, H, D, device)
+        pool.ts_kv_append(0, [sid], [3], dk, dk, TS_COMMIT)
+    q, k, v = (draw_bits_torch(gen, 3 * T, H, D, device) for _ in range(3))
+    out = torch.empty_like(q)
+    fn = lambda: pool.ts_chunk_step(0, [sid], [3], q, k, v, out, None, float(w.scale), 0)
+    for _ in range(3):
+        fn()
+    ts = _timed(fn, 20, device)
+    flops = synth.attention_flops(sh, w.sessions)
+    ms = float(np.median(ts))
+    pool.close()
+    return {"workload": "1 session x 12 heads, P=6, c=3 (444 query tiles on 148 SMs)", "ms_per_step": round(ms, 4),
+            "max_ms": round(max(ts), 4), "tflops": round(flops / ms / 1e9, 1), "frac": round(flops / ms / 1e9 / peak, 4)}
+
+
+def run_config3(device, peak):
+    """configs[3]: 4 sessions x 40 heads at the full window; one layer, and the 40-layer chunk step - 40 eager
+    ts_chunk_step calls against ONE CUDA graph of 40 ts_step_plan_run launches (NEXT-2)."""
+    import torch
+    import synth
+    from synth.draw import draw_bits_torch
+    from paper_2606_19271_b200 import TS_COMMIT, TS_RUN_APPEND, TurboChunkPool
+    torch.cuda.empty_cache()
+    free_b, _ = torch.cuda.mem_get_info(device)
+    NL = 40
+    w = synth.wan14b_batch(n_layers=NL)
+    sh = w.shape
+    per_layer = sh.n_pages * 2 * sh.n_heads * sh.page_tokens * sh.head_dim * 2
+    while NL > 1 and per_layer * NL + (6 << 30) > free_b:
+        NL //= 2
+    if NL != 40:
+        w = synth.wan14b_batch(n_layers=NL)
+        sh = w.shape
+    T, H, D = sh.frame_tokens, sh.n_heads, sh.head_dim
+    pool = TurboChunkPool(NL, H, D, sh.page_tokens, sh.n_pages, T, sh.window_frames, sh.max_sessions, device=device.index)
+    gen = torch.Generator(device=device)
+    gen.manual_seed(w.seed)
+    sids = [pool.ts_session_open() for _ in w.sessions]
+    cf = [3] * len(sids)
+    n_tok = 3 * T * len(sids)
+    for _ in range(0, 18, 3):
+        dk = draw_bits_torch(gen, n_tok, H, D, device)
+        dv = draw_bits_torch(gen, n_tok, H, D, device)
+        for layer in range(NL):
+            pool.ts_kv_append(layer, sids, cf, dk, dv, TS_COMMIT if layer == NL - 1 else 0)
+    q, k, v = (draw_bits_torch(gen, n_tok, H, D, device) for _ in range(3))
+    out = torch.empty_like(q)
+    scale = float(w.scale)
+    flops = synth.attention_flops(sh, w.sessions)
+    one = lambda: pool.ts_chunk_step(0, sids, cf, q, k, v, out, None, scale, 0)
+    for _ in range(2):
+        one()
+    t_one = _timed(one, 5, device)
+
+    def eager():
+        for layer in range(NL):
+            pool.ts_chunk_step(layer, sids, cf, q, k, v, out, None, scale, 0)
+    eager()
+    torch.cuda.synchronize(device)
+    host_eager, t_eager = [], []
+    for _ in range(3):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        h0 = time.perf_counter()
+        a.record()
+        eager()
+        b.record()
+        host_eager.append((time.perf_counter() - h0) * 1e3)
+        torch.cuda.synchronize(device)
+        t_eager.append(a.elapsed_time(b))
+    # the same step as one graph: prepare (host + one upload), one graph launch, commit
+    plan = pool.ts_step_plan_create(sids, cf, n_slots=1)
+    plan.ts_step_plan_bind(0, q, k, v, out, None)
+    stream = torch.cuda.Stream(device)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(stream):
+        plan.ts_step_plan_prepare(stream=stream)
+        stream.synchronize()
+        with torch.cuda.graph(graph, stream=stream, capture_error_mode="thread_local"):
+            for layer in range(NL):
+                plan.ts_step_plan_run(layer, 0, scale, TS_RUN_APPEND, stream=torch.cuda.current_stream())
+        graph.replay()
+        plan.ts_step_plan_commit(0, stream=stream)
+        stream.synchronize()
+        host_graph, t_graph = [], []
+        for _ in range(3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            h0 = time.perf_counter()
+            a.record(stream)
+            plan.ts_step_plan_prepare(stream=stream)
+            graph.replay()
+            plan.ts_step_plan_commit(0, stream=stream)
+            b.record(stream)
+            host_graph.append((time.perf_counter() - h0) * 1e3)
+            stream.synchronize()
+            t_graph.append(a.elapsed_time(b))
+    plan.close()
+    pool.close()
+    del pool, q, k, v, out
+    torch.cuda.empty_cache()
+    ms1 = float(np.median(t_one))
+    return {"workload": f"4 sessions x 40 heads, P=18 (full 21-frame window), {NL} layers"
+                        + ("" if NL == 40 else " (fewer than 40: not enough free HBM for the 107 GB slab)"),
+            "one_layer": {"ms": round(ms1, 4), "tflops": round(flops / ms1 / 1e9, 1), "frac": round(flops / ms1 / 1e9 / peak, 4)},
+            "chunk_step_eager": {"layers": NL, "calls": NL, "ms": round(min(t_eager), 2), "max_ms": round(max(t_eager), 2),
+                                 "host_ms": round(float(np.median(host_eager)), 3),
+                                 "tflops": round(flops * NL / min(t_eager) / 1e9, 1)},
+            "chunk_step_graph": {"layers": NL, "graph_launches": 1, "ms": round(min(t_graph), 2),
+                                 "max_ms": round(max(t_graph), 2), "host_ms": round(float(np.median(host_graph)), 3),
+                                 "tflops": round(flops * NL / min(t_graph) / 1e9, 1),
+                                 "frac": round(flops * NL / min(t_graph) / 1e9 / peak, 4),
+                                 "what": "ts_step_plan_prepare + cudaGraphLaunch(40 x ts_step_plan_run) + ts_step_plan_commit"}}
+
+
+def run_config4(device, peak):
+    """configs[4]: 200-step bursty churn (synth.churn_script, seed 4), Wan-1.3B attention shape, up to 32 sessions per step;
+    idle sessions suspended to the pinned arena and resumed on reactivation, all on the side stream.  Per-chunk latency =
+    wall clock from the first call of a step to the completion of its fused launch (a resume the batch waits for included)."""
+    import torch
+    import synth
+    from synth.draw import draw_bits_torch
+    from paper_2606_19271_b200 import TS_COMMIT, TurboChunkPool
+    T, H, D, B, Wn = 1560, 12, 128, 256, 21
+    steps = synth.churn_script()
+    rng = np.random.default_rng(4)
+    n_pages = 4000
+    pool = TurboChunkPool(1, H, D, B, n_pages, T, Wn, 128, free_order=rng.permutation(n_pages), host_pages=5400,
+                          device=device.index)
+    gen = torch.Generator(device=device)
+    gen.manual_seed(4)
+    C = 3 * T
+    cap = max(len(e["batch"]) for e in steps)
+    q, k, v = (draw_bits_torch(gen, cap * C, H, D, device) for _ in range(3))
+    out = torch.empty_like(q)
+    scale = float(1.0 / np.sqrt(D))
+    side = pool.side_stream
+    sid_of, frames = {}, {}
+    lat, flops, off_bytes, off_ms, n_served = [], [], 0, 0.0, []
+    for ev in steps:
+        torch.cuda.synchronize(device)
+        t0 = time.perf_counter()
+        moved = 0
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(side)
+        for u in ev["suspend"]:
+            moved += pool.ts_session_info(sid_of[u])["n_pages"] * pool.page_bytes
+            pool.ts_session_suspend(sid_of[u])
+        for u in ev["resume"]:
+            pool.ts_session_resume(sid_of[u])
+            moved += pool.ts_session_info(sid_of[u])["n_pages"] * pool.page_bytes
+        s1.record(side)
+        for u in ev["open"]:
+            sid_of[u] = pool.ts_session_open()
+            frames[u] = 0
+        batch = [sid_of[u] for u in ev["batch"]]
+        if batch:
+            n_tok = len(batch) * C
+            pool.ts_chunk_step(0, batch, ev["chunk_frames"], q[:n_tok], k[:n_tok], v[:n_tok], out[:n_tok], None, scale, TS_COMMIT)
+            torch.cuda.current_stream().synchronize()
+            lat.append((time.perf_counter() - t0) * 1e3)
+            flops.append(4 * D * H * sum(synth.attention_pairs(frames[u], 3, T, Wn) for u in ev["batch"]))
+            n_served.append(len(batch))
+            for u in ev["batch"]:
+                frames[u] = min(Wn, frames[u] + 3)
+        torch.cuda.synchronize(device)
+        if moved:
+            off_bytes += moved
+            off_ms += s0.elapsed_time(s1)
+        for u in ev["close"]:
+            pool.ts_session_close(sid_of.pop(u))
+            frames.pop(u)
+    pool.close()
+    lat_a, fl = np.array(lat), np.array(flops)
+    return {"workload": "200-step MMPP churn (mean 4 / 24 sessions, cap 32), suspend/resume through pinned host memory",
+            "served_steps": len(lat), "max_batch": int(max(n_served)), "latency_ms_p50": round(float(np.median(lat_a)), 3),
+            "latency_ms_p99": round(float(np.percentile(lat_a, 99)), 3), "latency_ms_max": round(float(lat_a.max()), 3),
+            "attention_tflops": round(float(fl.sum() / lat_a.sum() / 1e9), 1),
+            "attention_tflops_best_step": round(float((fl / lat_a).max() / 1e9), 1),
+            "frac": round(float(fl.sum() / lat_a.sum() / 1e9) / peak, 4),
+            "offload_gb": round(off_bytes / 1e9, 2), "offload_gbs": round(off_bytes / max(off_ms, 1e-9) / 1e6, 2),
+            "note": "latency includes the host calls and any resume the batch waits for; offload rate = bytes / side-stream time"}
 
 
 def measure_offload(wl, permuted=False):
@@ -459,7 +966,7 @@ def measure_migration(wl, hbm_peak):
     """ts_session_migrate of a full-window (21-frame) session between two pools, ping-pong, 8 moves enqueued back to
     back behind a blocker copy (so that the host's enqueue time is not in the events).  Both pools sit on this one GPU,
     where the fetch kernel is HBM-bound (read + write of the session's pages); between two GPUs the same kernel reads
-    the source slab over NVLink - not measurable on a 1-GPU box."""
+    the source slab over NVLink (`migrate_p2p`, --gpus >= 2)."""
     import torch
     from synth.draw import draw_bits_torch
     from paper_2606_19271_b200 import TS_COMMIT, TurboChunkPool
@@ -500,7 +1007,48 @@ def measure_migration(wl, hbm_peak):
             "note": "both pools on this GPU (read + write in HBM); across GPUs the fetch reads over NVLink"}
 
 
-def run_reference(args):
+def measure_migration_p2p(wl, peer_peak_gbs=770.0):
+    """--gpus >= 2, rank 0 only (the other ranks wait at a barrier): a full-window session moved between a pool on device 0
+    and a pool on device 1 of THIS process, both ways.  The fetch kernel runs on the target and reads the source slab
+    through the peer mapping (NVLink); timed by events on the target's side stream."""
+    import torch
+    from synth.draw import draw_bits_torch
+    from paper_2606_19271_b200 import TS_COMMIT, TurboChunkPool
+    sh = wl["w"].shape
+    T, H, D = sh.frame_tokens, sh.n_heads, sh.head_dim
+    pools = [TurboChunkPool(1, H, D, sh.page_tokens, 160, T, sh.window_frames, 2, device=d) for d in (0, 1)]
+    dev0 = torch.device("cuda", 0)
+    gen = torch.Generator(device=dev0)
+    gen.manual_seed(98)
+    with torch.cuda.device(0):
+        sid = pools[0].ts_session_open()
+        for _ in range(7):
+            kk = draw_bits_torch(gen, 3 * T, H, D, dev0)
+            pools[0].ts_kv_append(0, [sid], [3], kk, kk, TS_COMMIT)
+    nbytes = pools[0].ts_session_info(sid)["n_pages"] * pools[0].page_bytes
+    torch.cuda.synchronize(0)
+    times = []
+    for i in range(8):
+        src, dst = pools[i & 1], pools[(i & 1) ^ 1]
+        with torch.cuda.device((i & 1) ^ 1):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(dst.side_stream)
+            sid = src.ts_session_migrate(sid, dst)
+            b.record(dst.side_stream)
+            dst.side_stream.synchronize()
+            times.append(a.elapsed_time(b))
+    for p in pools:
+        p.close()
+    torch.cuda.set_device(0)
+    best = float(np.min(times[2:]))
+    gbs = nbytes / (best * 1e-3) / 1e9
+    return {"bound": "nvlink", "kernel": "page_pull_kernel (peer loads)", "bytes_moved": int(nbytes),
+            "ms_per_move": round(best, 4), "achieved": round(gbs, 1), "peak": peer_peak_gbs, "unit": "GB/s",
+            "frac": round(gbs / peer_peak_gbs, 4),
+            "peak_kind": "measured peer copy on this pool, 770 GB/s per direction (B200_PROFILING.md); nominal 900"}
+
+
+def run_reference(args, world):
     """The CPU oracle as it stands, on the same config/metric; each step is a bounded sample of the workload.
     Inputs are drawn on the host (numpy path of synth/) so that this arm needs no GPU."""
     import oracle
@@ -508,6 +1056,7 @@ def run_reference(args):
     w = synth.wan13b_batch()
     sh = w.shape
     T, H, D = sh.frame_tokens, sh.n_heads, sh.head_dim
+    cfg = config_dict(w, world)
     opool = oracle.OraclePool(sh.n_layers, H, D, sh.page_tokens, sh.n_pages, T, sh.window_frames, sh.max_sessions,
                               w.free_order)
     sids, chunk_bits = [], []
@@ -517,20 +1066,27 @@ def run_reference(args):
             opool.append(0, [sid], [3], synth.draw_bits(w.rng, 3 * T, H, D), synth.draw_bits(w.rng, 3 * T, H, D))
         chunk_bits.append(tuple(synth.draw_bits(w.rng, 3 * T, H, D) for _ in range(3)))
         sids.append(sid)
-    steps = max(1, min(args.steps, 3))
-    oracle_sample(w, opool, sids, chunk_bits)          # warm-up
-    tot_t, tot_f, desc = 0.0, 0, ""
-    for _ in range(steps):
-        dt, fl, desc = oracle_sample(w, opool, sids, chunk_bits)
-        tot_t += dt
-        tot_f += fl
+    steps, warmup = max(1, args.steps), max(1, args.warmup)
+    # each step = a bounded sample of the workload, sized so that warmup + steps end within a few minutes: one whole head
+    # of as many sessions as a per-step budget allows (the batch's sessions in order, wrapping around)
+    t_probe, _, _ = oracle_sample(w, opool, sids[:1], chunk_bits[:1])
+    budget_s = 150.0 / (steps + warmup)
+    per_step = int(max(1, min(len(sids), budget_s / max(t_probe, 1e-3))))
+    tot_t, tot_f, desc, cursor = 0.0, 0, "", 0
+    for it in range(warmup + steps):
+        pick = [(cursor + j) % len(sids) for j in range(per_step)]
+        cursor += per_step
+        dt, fl, desc = oracle_sample(w, opool, [sids[j] for j in pick], [chunk_bits[j] for j in pick])
+        if it >= warmup:
+            tot_t += dt
+            tot_f += fl
     value = tot_f / tot_t / 1e12
+    sample = f"per step: one whole head (all 4680 query rows over all visible keys) of {per_step} of the 8 sessions, fp64 numpy"
     print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": round(value, 5), "unit": UNIT, "n_gpus": 1, "steps": steps,
-        "warmup": 1, "ms_per_step": round(tot_t / steps * 1e3, 2), "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "prior_frames": [s.prior_frames for s in w.sessions]},
-        "cpu_baseline": {"value": round(value, 5), "unit": UNIT, "kind": "oracle", "cores": cpu_threads(), "sample": desc},
+        "impl": "reference", "metric": METRIC, "value": round(value, 5), "unit": UNIT, "n_gpus": world, "steps": steps,
+        "warmup": warmup, "ms_per_step": round(tot_t / steps * 1e3, 2), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
+        "cpu_baseline": {"value": round(value, 5), "unit": UNIT, "kind": "oracle", "cores": cpu_threads(), "sample": sample},
         "e2e": {"value": round(value, 5), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 

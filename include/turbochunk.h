@@ -283,6 +283,14 @@ void* ts_pool_side_stream(ts_pool* pool);
 /* Number of kernels the library has launched on this pool since creation (bench.py's gpu_launches). */
 int64_t ts_pool_launch_count(ts_pool* pool);
 
+/* Number of times the ragged batch scheduler (a1) had to build a schedule (the rest were reuses of the cached one). */
+int64_t ts_pool_sched_builds(ts_pool* pool);
+/* Measurement aid: while `device_u64x2` (device, 8-byte aligned, caller-zeroed) is set, CTA 0 of every attention
+ * launch (captured launches: those recorded while it was set) adds the SM cycles and the nanoseconds it ran for to
+ * [0] and [1]; [0] / [1] is the SM clock in GHz under the kernel itself, which a host-side sampler cannot see.
+ * NULL switches it off.  Launches must not overlap while it is on. */
+int ts_pool_clock_probe(ts_pool* pool, void* device_u64x2);
+
 const char* ts_strerror(int code);
 /* Text of the last CUDA error seen by this pool's calls on this thread ("" if none). */
 const char* ts_last_cuda_error(void);

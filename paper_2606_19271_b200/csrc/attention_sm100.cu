@@ -73,7 +73,7 @@ struct Cfg {
   static constexpr int kSmemKV = kSlots * kTileBytes;
   static constexpr int kNumBars = 2 * kSlots + 2 + 10;
   static constexpr int kXchgBytes = 2 * 128 * 2 * 4;    // (m, l) of a row from each softmax warpgroup (lone-tile merge)
-  static constexpr int kSmemBytes = kSmemQ + kSmemKV + kXchgBytes + kNumBars * 8 + 16;
+  static constexpr int kSmemBytes = kSmemQ + kSmemKV + kXchgBytes + kNumBars * 8 + 16 + 16;   // + TMEM base, clock-probe stamps
 };
 
 struct ItemGeom {
@@ -196,6 +196,15 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
   tc_fence_after();
   const uint32_t cta_rank = cluster_ctarank();
   const uint32_t tmem_base = *tmem_ptr;
+  // optional in-kernel clock probe (one thread of CTA 0, a warp without a role on the critical path)
+  // (the start stamps wait in shared memory: no register lives across the kernel for it)
+  unsigned long long* probe_smem = reinterpret_cast<unsigned long long*>(tmem_ptr + 4);
+  if (p.clock_probe != nullptr && blockIdx.x == 0 && threadIdx.x == 96) {
+    unsigned long long ns0;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns0));
+    probe_smem[0] = (unsigned long long)clock64();
+    probe_smem[1] = ns0;
+  }
 
 
   if (warp < 4) {
@@ -630,6 +639,13 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
   __syncthreads();
   cluster_sync_all();   // no CTA exits while its partner may still multicast into it or arrive on its barriers
   if (warp == 1) tmem_dealloc(tmem_base, kTmemCols);
+  if (p.clock_probe != nullptr && blockIdx.x == 0 && threadIdx.x == 96) {
+    unsigned long long ns1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns1));
+    const unsigned long long* probe_smem = reinterpret_cast<const unsigned long long*>(tmem_ptr + 4);
+    p.clock_probe[0] += (unsigned long long)clock64() - probe_smem[0];
+    p.clock_probe[1] += ns1 - probe_smem[1];
+  }
   // every role of both CTAs has read the ring's last entry: clear it for the next launch on this block
   if (cta_rank == 0 && threadIdx.x >= 64 && threadIdx.x < 64 + kFeedRing)
     p.feed[(size_t)(blockIdx.x >> 1) * kFeedRing + (threadIdx.x - 64)] = 0ull;

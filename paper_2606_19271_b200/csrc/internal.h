@@ -90,6 +90,8 @@ struct AttnParams {
   int32_t H, T, B, log2_B;
   float scale_log2;              // scale * log2(e)
   float scale;
+  unsigned long long* clock_probe;  // null, or device uint64[2]: CTA 0 adds the SM cycles (clock64) and the nanoseconds
+                                 // (globaltimer) it ran for, so that sum cycles / sum ns is the SM clock under THIS kernel
   CopyParams copy;               // fused chunk step: the KV append, done by the two idle warps of every CTA
                                  // (copy.n_sess == 0: none)
 };
@@ -99,6 +101,7 @@ cudaError_t launch_attention(const AttnParams& p, int head_dim, int grid, cudaSt
 cudaError_t launch_append(const CopyParams& p, int sm_count, cudaStream_t stream);
 cudaError_t launch_gather(const CopyParams& p, int sm_count, cudaStream_t stream);
 cudaError_t launch_page_pull(const PullParams& p, int sm_count, cudaStream_t stream);
+cudaError_t launch_upload(const void* src_mapped, void* dst, size_t bytes, cudaStream_t stream);
 int attention_smem_bytes(int head_dim);
 cudaError_t attention_configure(int head_dim);   // sets the kernel's dynamic shared memory limit on the current device (idempotent)
 

@@ -101,6 +101,40 @@ cudaError_t launch_page_pull(const PullParams& p, int sm_count, cudaStream_t str
   return cudaGetLastError();
 }
 
+// Descriptor upload without a copy engine.  Per-call schedule / descriptor blocks (tens of KB) are pulled from mapped
+// pinned host memory by a few warps instead of a cudaMemcpyAsync: a DMA copy queues behind whatever the copy engine is
+// already moving - a 201 MB resume on the side stream delayed a 2.45 ms step by 4.2 ms that way (bench.py `overlap`).
+// ld.cv: system-memory lines are never served from a stale cache line (the host rewrites the staging ring).
+constexpr int kUploadThreads = 64;
+constexpr int kUploadUnroll = 4;
+
+__global__ void __launch_bounds__(kUploadThreads) upload_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, int n_vec) {
+  const int stride = gridDim.x * kUploadThreads;
+  for (int e0 = blockIdx.x * kUploadThreads + threadIdx.x; e0 < n_vec; e0 += stride * kUploadUnroll) {
+    uint4 r[kUploadUnroll];
+#pragma unroll
+    for (int u = 0; u < kUploadUnroll; ++u) {
+      const int e = e0 + u * stride;
+      if (e < n_vec)
+        asm volatile("ld.global.cv.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r[u].x), "=r"(r[u].y), "=r"(r[u].z), "=r"(r[u].w) : "l"(src + e));
+    }
+#pragma unroll
+    for (int u = 0; u < kUploadUnroll; ++u) {
+      const int e = e0 + u * stride;
+      if (e < n_vec) dst[e] = r[u];
+    }
+  }
+}
+
+// bytes: a multiple of 16; src_mapped: the device-side address of mapped pinned host memory
+cudaError_t launch_upload(const void* src_mapped, void* dst, size_t bytes, cudaStream_t stream) {
+  const int n_vec = (int)(bytes / 16);
+  int grid = (n_vec + kUploadThreads * kUploadUnroll - 1) / (kUploadThreads * kUploadUnroll);
+  grid = grid < 1 ? 1 : (grid > 32 ? 32 : grid);
+  upload_kernel<<<grid, kUploadThreads, 0, stream>>>(reinterpret_cast<const uint4*>(src_mapped), reinterpret_cast<uint4*>(dst), n_vec);
+  return cudaGetLastError();
+}
+
 static dim3 copy_grid(const CopyParams& p, int sm_count, int64_t max_vecs_per_sess) {
   // enough CTAs to fill the machine (8 resident CTAs of 256 threads per SM), split evenly over sessions
   int64_t want = (max_vecs_per_sess + (int64_t)kCopyThreads * kCopyUnroll - 1) / ((int64_t)kCopyThreads * kCopyUnroll);

@@ -113,8 +113,9 @@ struct Session {
   bool in_plan = false;             // between ts_step_plan_prepare and ts_step_plan_commit: no other call may touch it
 };
 
-struct Staging {      // pinned host + device buffer pair for per-call schedule records
+struct Staging {      // pinned (mapped) host + device buffer pair for per-call schedule records
   uint8_t* h = nullptr;
+  uint8_t* h_dev = nullptr;      // the device-side address of `h` (what the upload kernel reads)
   uint8_t* d = nullptr;
   size_t cap = 0;
   cudaEvent_t ev = nullptr;      // recorded on the consumer's stream after the kernel that reads `d`
@@ -168,6 +169,7 @@ struct ts_pool {
   std::vector<int32_t> sched_pt, sched_cta;
   std::vector<tc::WorkItem> sched_items;
   int64_t sched_builds = 0;
+  unsigned long long* clock_probe = nullptr;   // ts_pool_clock_probe
 };
 
 namespace tc {
@@ -198,7 +200,8 @@ static int acquire_staging(ts_pool* pool, size_t bytes, Staging** out) {
     s.h = s.d = nullptr;
     s.cap = 0;
     const size_t cap = align_up(std::max(bytes * 2, (size_t)65536), 4096);
-    TS_CUDA(cudaHostAlloc((void**)&s.h, cap, cudaHostAllocDefault));
+    TS_CUDA(cudaHostAlloc((void**)&s.h, cap, cudaHostAllocMapped));
+    TS_CUDA(cudaHostGetDevicePointer((void**)&s.h_dev, s.h, 0));
     TS_CUDA(cudaMalloc((void**)&s.d, cap));
     s.cap = cap;
   }
@@ -207,11 +210,16 @@ static int acquire_staging(ts_pool* pool, size_t bytes, Staging** out) {
 }
 
 // The per-call descriptor block does not depend on anything the caller's stream is doing: it is uploaded on the pool's
-// own stream, so that the copy runs under the previous kernel instead of between two kernels of the caller's stream,
-// which only waits for the (normally long complete) upload event.
+// own (high-priority) stream, so that the copy runs under / in the tail of the previous kernel instead of between two
+// kernels of the caller's stream, which only waits for the (normally long complete) upload event.  The copy is a small
+// kernel reading mapped pinned memory, never a DMA copy: those queue behind the offload traffic of the copy engines.
 static int upload_staging(ts_pool* pool, Staging* st, size_t bytes, cudaStream_t consumer) {
-  if (pool->up_s == nullptr) TS_CUDA(cudaStreamCreateWithFlags(&pool->up_s, cudaStreamNonBlocking));
-  TS_CUDA(cudaMemcpyAsync(st->d, st->h, bytes, cudaMemcpyHostToDevice, pool->up_s));
+  if (pool->up_s == nullptr) {
+    int lo = 0, hi = 0;
+    TS_CUDA(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+    TS_CUDA(cudaStreamCreateWithPriority(&pool->up_s, cudaStreamNonBlocking, hi));
+  }
+  TS_CUDA(launch_upload(st->h_dev, st->d, align_up(bytes, 16), pool->up_s));
   TS_CUDA(cudaEventRecord(st->ev_up, pool->up_s));
   TS_CUDA(cudaStreamWaitEvent(consumer, st->ev_up, 0));
   return TS_OK;
@@ -524,6 +532,12 @@ int ts_pool_stats(ts_pool* pool, ts_pool_stats_t* out) {
 }
 
 void* ts_pool_side_stream(ts_pool* pool) { return pool ? (void*)pool->side : nullptr; }
+int64_t ts_pool_sched_builds(ts_pool* pool) { return pool ? pool->sched_builds : 0; }
+int ts_pool_clock_probe(ts_pool* pool, void* device_u64x2) {
+  if (pool == nullptr || ((uintptr_t)device_u64x2 & 7) != 0) return TS_ERR_INVALID;
+  pool->clock_probe = (unsigned long long*)device_u64x2;
+  return TS_OK;
+}
 int64_t ts_pool_launch_count(ts_pool* pool) { return pool ? pool->launches : 0; }
 
 // --------------------------------------------------------------------------------------------- a1: schedule
@@ -777,6 +791,7 @@ static AttnParams make_params(ts_pool* pool, const BlockLayout& L, uint8_t* d, i
   p.sess_maps = reinterpret_cast<const CUtensorMap*>(d + L.off_maps) + (size_t)slot * n * 3;
   p.sess = reinterpret_cast<const SessDesc*>(d + L.off_sess);
   p.page_tables = reinterpret_cast<const int32_t*>(d + L.off_pt);
+  p.clock_probe = pool->clock_probe;
   p.feed_hdr = reinterpret_cast<int32_t*>(d + L.off_feed);
   p.feed = reinterpret_cast<unsigned long long*>(d + L.off_feed + 128);
   p.items = reinterpret_cast<const WorkItem*>(d + L.off_items);
@@ -1079,6 +1094,7 @@ struct ts_step_plan {
   size_t max_pt = 0, max_items = 0;
   uint8_t* d = nullptr;              // device block: its address never changes, so captured launches stay valid
   uint8_t* h[2] = {nullptr, nullptr};
+  uint8_t* h_dev[2] = {nullptr, nullptr};   // device-side addresses of the mapped pinned buffers
   cudaEvent_t h_ev[2] = {nullptr, nullptr};
   bool h_busy[2] = {false, false};
   int h_next = 0;
@@ -1142,11 +1158,12 @@ int ts_step_plan_create(ts_pool* pool, int32_t n, const int32_t* sids, const int
     ts_step_plan_destroy(plan);
     return code;
   };
-  if (!cuda_ok(cudaMalloc((void**)&plan->d, plan->L.bytes), "cudaMalloc(step plan)")) return fail(TS_ERR_CUDA);
+  if (!cuda_ok(cudaMalloc((void**)&plan->d, align_up(plan->L.bytes, 16)), "cudaMalloc(step plan)")) return fail(TS_ERR_CUDA);
   if (!cuda_ok(cudaMemset(plan->d, 0, plan->L.bytes), "cudaMemset(step plan)")) return fail(TS_ERR_CUDA);
   for (int i = 0; i < 2; ++i) {
-    if (!cuda_ok(cudaHostAlloc((void**)&plan->h[i], plan->L.bytes, cudaHostAllocDefault), "cudaHostAlloc(step plan)"))
+    if (!cuda_ok(cudaHostAlloc((void**)&plan->h[i], align_up(plan->L.bytes, 16), cudaHostAllocMapped), "cudaHostAlloc(step plan)"))
       return fail(TS_ERR_CUDA);
+    if (!cuda_ok(cudaHostGetDevicePointer((void**)&plan->h_dev[i], plan->h[i], 0), "cudaHostGetDevicePointer")) return fail(TS_ERR_CUDA);
     if (!cuda_ok(cudaEventCreateWithFlags(&plan->h_ev[i], cudaEventDisableTiming), "cudaEventCreate")) return fail(TS_ERR_CUDA);
   }
   if (!cuda_ok(attention_configure(c.head_dim), "cudaFuncSetAttribute(attention)")) return fail(TS_ERR_CUDA);
@@ -1204,7 +1221,7 @@ int ts_step_plan_prepare(ts_step_plan* plan, void* cuda_stream) {
   if (e == cudaSuccess) e = pool->tl_side.wait(stream, fa.wait_side);
   if (e == cudaSuccess) e = pool->tl_compute.wait(stream, fa.wait_compute);
   // the block is rewritten in stream order: after the previous step's launches, before this step's
-  if (e == cudaSuccess) e = cudaMemcpyAsync(plan->d, h, plan->L.bytes, cudaMemcpyHostToDevice, stream);
+  if (e == cudaSuccess) e = launch_upload(plan->h_dev[slot], plan->d, align_up(plan->L.bytes, 16), stream);
   if (e == cudaSuccess) e = cudaEventRecord(plan->h_ev[slot], stream);
   if (!cuda_ok(e, "ts_step_plan_prepare")) {
     ungrow(pool, n, sids, fa);
@@ -1445,7 +1462,7 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
     TS_CUDA_UNDO(src->tl_compute.wait(dst->side, s.compute_seq));
     TS_CUDA_UNDO(src->tl_side.wait(dst->side, s.side_seq));
     TS_CUDA_UNDO(dst->tl_compute.wait(dst->side, wait_compute));
-    TS_CUDA_UNDO(cudaMemcpyAsync(st->d, st->h, n * 8, cudaMemcpyHostToDevice, dst->side));
+    TS_CUDA_UNDO(launch_upload(st->h_dev, st->d, align_up(n * 8, 16), dst->side));   // not a DMA copy: see upload_staging
     PullParams p;
     p.src_slab = src->slab;
     p.dst_slab = dst->slab;

@@ -31,7 +31,21 @@ def test_bench_line_contract():
     assert r["bound"] == "tensor" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-3
     assert r["traffic"] is None or r["traffic"] > 0
     assert 0.3 < r["frac"] < 1.0 and d["value"] > 500
-    assert d["gpu_launches"] == 4                                   # one fused launch per timed step
+    assert d["gpu_launches"] == 5                                   # one fused launch per timed step + one committed step
+    assert r["ms_per_launch"] <= d["ms_per_step"]                   # the roofline comes from the timed loop itself
+    assert d["step"]["sched_builds_in_timed_loop"] >= 2             # a1 is inside timed steps, not only the cached reuse
+    assert 1000 < d["clocks"]["sm_mhz_in_kernel"] <= d["clocks"]["sm_max_mhz"] + 50
+    s = d["sustained"]
+    assert s["seconds"] >= 2.0 and 0.3 < s["frac"] < 1.1 and s["sm_mhz_in_kernel"] > 1000
+    o = d["overlap"]
+    assert 0.9 * o["step_alone_ms"] <= o["step_with_offload_ms"] <= 1.5 * o["step_alone_ms"] and o["resume_h2d_gbs_under_load"] > 10
+    lm = d["latency_model"]
+    assert [x["n"] for x in lm["l_hat"]] == [1, 2, 4, 5, 6, 8, 16, 32] and lm["largest_n_under_slo"] >= 1
+    cfgs = d["configs"]
+    assert set(cfgs) == {"configs[1]", "configs[3]", "configs[4]"}
+    assert cfgs["configs[3]"]["chunk_step_graph"]["graph_launches"] == 1
+    assert cfgs["configs[3]"]["chunk_step_graph"]["ms"] <= 1.05 * cfgs["configs[3]"]["chunk_step_eager"]["ms"]
+    assert cfgs["configs[4]"]["served_steps"] > 150 and cfgs["configs[4]"]["latency_ms_max"] >= cfgs["configs[4]"]["latency_ms_p50"]
     e = d["e2e"]
     assert e["h2d_bytes_per_step"] > 3e8 and e["d2h_bytes_per_step"] > 1e8 and 0 < e["value"] < d["value"]
     c = d["cpu_baseline"]
@@ -44,6 +58,9 @@ def test_bench_line_contract():
 
 
 def test_reference_arm_line():
-    d = run("--impl", "reference", "--steps", "1", "--warmup", "1")
+    d = run("--impl", "reference", "--steps", "2", "--warmup", "1")
     assert d["impl"] == "reference" and d["dtype"] == "f64" and d["value"] > 0
+    assert d["steps"] == 2 and d["warmup"] == 1                     # the arm honours --steps / --warmup
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+    ours = run("--steps", "3", "--warmup", "3", "--no-extras")
+    assert ours["config"] == d["config"]                            # both arms describe the workload identically
