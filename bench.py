@@ -301,6 +301,9 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--power-table", action="store_true",
+                    help="print the clock / power table of profiles/r2_power_table.md (attention kernel vs cuBLAS bf16, burst "
+                         "and sustained) instead of the bench line")
     ap.add_argument("--no-extras", action="store_true",
                     help="only the timed loop, the roofline and e2e (skips sustained / configs / overlap / latency_model)")
     args = ap.parse_args()
@@ -328,6 +331,9 @@ def main():
     peaks, peaks_kind = load_peaks()
     extras = (world == 1) and not args.no_extras
 
+    if args.power_table:
+        print(json.dumps(power_table(device, peaks), indent=1))
+        return 0
     wl = build_workload(device, with_oracle=(rank == 0 and world == 1))
     pool, w = wl["pool"], wl["w"]
     sh = w.shape
@@ -492,6 +498,112 @@ def main():
     if world > 1:
         torch.distributed.barrier()
     return 0
+
+
+# ------------------------------------------------------------------------------------------------ power table
+class PowerSampler(ClockSampler):
+    """ClockSampler that also records board power (NVML, mW)."""
+
+    def _run(self):
+        nv = self.nv
+        self.power = []
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1e3)
+                mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                if mask & getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4):
+                    self.reasons.add("sw_power_cap")
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+
+def power_table(device, peaks):
+    """What bounds the attention kernel on this box: SM clock under the kernel (in-kernel probe), SM cycles per launch
+    (independent of the clock), board power, against cuBLAS bf16 8192^3 in the same two regimes (burst: 20 launches after
+    an idle second; sustained: back to back for 3 s)."""
+    import torch
+    import synth
+    wl = build_workload(device, False)
+    pool, w = wl["pool"], wl["w"]
+    flops = synth.attention_flops(w.shape, w.sessions)
+    out = torch.empty_like(wl["q"])
+    scale = float(w.scale)
+    probe = torch.zeros(2, dtype=torch.int64, device=device)
+    idx = device.index or 0
+    peak_per_mhz = 148 * 8192 / 1e6            # TFLOP/s per MHz of SM clock at 100 % tensor-pipe activity (8192 FLOP/clk/SM)
+
+    def attn():
+        pool.ts_chunk_attention(0, wl["sids"], wl["cf"], wl["q"], wl["k"], wl["v"], out, None, scale)
+
+    a = torch.randn(8192, 8192, device=device, dtype=torch.bfloat16)
+    b = torch.randn(8192, 8192, device=device, dtype=torch.bfloat16)
+    c = torch.empty_like(a)
+    mm_flops = 2 * 8192 ** 3
+
+    def mm():
+        torch.matmul(a, b, out=c)
+
+    def run(fn, fl, n=None, seconds=None, probe_on=False):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize(device)
+        time.sleep(1.0)
+        if probe_on:
+            probe.zero_()
+            pool.ts_pool_clock_probe(probe)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        count = 0
+        with PowerSampler(idx, period=0.005) as ps:
+            e0.record()
+            if n is not None:
+                for _ in range(n):
+                    fn()
+                count = n
+            else:
+                t0 = time.perf_counter()
+                while time.perf_counter() - t0 < seconds:
+                    for _ in range(50):
+                        fn()
+                    count += 50
+                    torch.cuda.synchronize(device)
+            e1.record()
+            torch.cuda.synchronize(device)
+        ms = e0.elapsed_time(e1)
+        row = {"launches": count, "ms_per_launch": round(ms / count, 4), "tflops": round(fl * count / ms / 1e9, 1),
+               "nvml_sm_mhz_median": float(np.median(ps.samples)) if ps.samples else None,
+               "nvml_power_w_median": round(float(np.median(ps.power)), 1) if ps.power else None,
+               "nvml_power_w_max": round(float(np.max(ps.power)), 1) if ps.power else None,
+               "reasons": sorted(ps.reasons)}
+        if probe_on:
+            pool.ts_pool_clock_probe(None)
+            cyc, ns = (int(x) for x in probe.tolist())
+            mhz = cyc / ns * 1e3
+            row.update({"sm_mhz_in_kernel": round(mhz, 1), "mcycles_per_launch": round(cyc / count / 1e6, 4),
+                        "tensor_pipe_floor_mcycles": round(fl / (148 * 8192) / 1e6, 4),
+                        "tensor_frac_of_cycles": round(fl / (148 * 8192) / (cyc / count), 4),
+                        "peak_at_this_clock_tflops": round(peak_per_mhz * mhz, 1)})
+        else:
+            # cuBLAS cannot be probed from inside: the clock it must at least have run at, were its tensor pipe 100 % active
+            row["implied_min_sm_mhz"] = round(row["tflops"] / peak_per_mhz, 1)
+        if row["nvml_power_w_median"]:
+            row["joule_per_launch"] = round(row["nvml_power_w_median"] * ms / count / 1e3, 3)
+            row["pj_per_flop"] = round(row["nvml_power_w_median"] * ms * 1e-3 / (fl * count) * 1e12, 3)
+        return row
+
+    table = {"workload": WORKLOAD + " (attention-only launches, 3.14 TFLOP each)",
+             "attention_burst_20": run(attn, flops, n=20, probe_on=True),
+             "attention_sustained_3s": run(attn, flops, seconds=3.0, probe_on=True),
+             "cublas_bf16_8192_burst_20": run(mm, mm_flops, n=20),
+             "cublas_bf16_8192_sustained_3s": run(mm, mm_flops, seconds=3.0),
+             "measured_peaks": {k: peaks.get(k) for k in ("bf16_tflops", "bf16_tflops_sustained")}}
+    tgt = 0.6 * NOMINAL_BF16_TFLOPS
+    for key in ("attention_burst_20", "attention_sustained_3s"):
+        r = table[key]
+        r["tensor_frac_needed_for_1350_at_this_clock"] = round(tgt / r["peak_at_this_clock_tflops"], 4)
+    pool.close()
+    return table
 
 
 # ------------------------------------------------------------------------------------------------ legs

@@ -142,9 +142,9 @@ def _ptr(t):
     return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
 
 
-def _stream(stream):
+def _stream(stream, device=None):
     if stream is None:
-        stream = torch.cuda.current_stream()
+        stream = torch.cuda.current_stream(device)      # the current stream of the POOL's device, not of the current device
     return C.c_void_p(stream.cuda_stream)
 
 
@@ -251,23 +251,23 @@ class TurboChunkPool:
     # ---- hot path
     def ts_chunk_attention(self, layer, sids, chunk_frames, q, k, v, out, lse=None, scale=1.0, stream=None):
         _check(lib.ts_chunk_attention(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(q), _ptr(k),
-                                      _ptr(v), _ptr(out), _ptr(lse), C.c_float(float(scale)), _stream(stream)),
+                                      _ptr(v), _ptr(out), _ptr(lse), C.c_float(float(scale)), _stream(stream, self.device)),
                "ts_chunk_attention")
 
     def ts_kv_append(self, layer, sids, chunk_frames, k, v, flags=TS_COMMIT, stream=None):
         _check(lib.ts_kv_append(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(k), _ptr(v),
-                                C.c_uint32(flags), _stream(stream)), "ts_kv_append")
+                                C.c_uint32(flags), _stream(stream, self.device)), "ts_kv_append")
 
     def ts_chunk_step(self, layer, sids, chunk_frames, q, k, v, out, lse=None, scale=1.0, flags=TS_COMMIT, stream=None):
         _check(lib.ts_chunk_step(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(q), _ptr(k), _ptr(v),
-                                 _ptr(out), _ptr(lse), C.c_float(float(scale)), C.c_uint32(flags), _stream(stream)),
+                                 _ptr(out), _ptr(lse), C.c_float(float(scale)), C.c_uint32(flags), _stream(stream, self.device)),
                "ts_chunk_step")
 
     def ts_chunk_step_host(self, layer, sids, chunk_frames, q_host, k_host, v_host, out_host, scale, flags=TS_COMMIT,
                            stream=None):
         _check(lib.ts_chunk_step_host(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(q_host),
                                       _ptr(k_host), _ptr(v_host), _ptr(out_host), C.c_float(float(scale)),
-                                      C.c_uint32(flags), _stream(stream)), "ts_chunk_step_host")
+                                      C.c_uint32(flags), _stream(stream, self.device)), "ts_chunk_step_host")
 
     def ts_step_plan_create(self, sids, chunk_frames, n_slots=1):
         """A capture-safe multi-layer step plan for this batch (include/turbochunk.h); returns a StepPlan."""
@@ -314,7 +314,7 @@ class TurboChunkPool:
         H, D = self.shape[1], self.shape[2]
         k = torch.empty((info["len_tokens"], H, D), dtype=torch.bfloat16, device=self.device)
         v = torch.empty_like(k)
-        _check(lib.ts_gather_kv(self._h, layer, sid, _ptr(k), _ptr(v), _stream(stream)), "ts_gather_kv")
+        _check(lib.ts_gather_kv(self._h, layer, sid, _ptr(k), _ptr(v), _stream(stream, self.device)), "ts_gather_kv")
         return k, v
 
     def ts_pool_stats(self):
@@ -352,14 +352,14 @@ class StepPlan:
         self._keep[slot] = (q, k, v, out, lse)
 
     def ts_step_plan_prepare(self, stream=None):
-        _check(lib.ts_step_plan_prepare(self._h, _stream(stream)), "ts_step_plan_prepare")
+        _check(lib.ts_step_plan_prepare(self._h, _stream(stream, self._pool.device)), "ts_step_plan_prepare")
 
     def ts_step_plan_run(self, layer, slot, scale, run_flags=TS_RUN_APPEND, stream=None):
-        _check(lib.ts_step_plan_run(self._h, layer, slot, C.c_float(float(scale)), C.c_uint32(run_flags), _stream(stream)),
+        _check(lib.ts_step_plan_run(self._h, layer, slot, C.c_float(float(scale)), C.c_uint32(run_flags), _stream(stream, self._pool.device)),
                "ts_step_plan_run")
 
     def ts_step_plan_commit(self, flags=TS_COMMIT, stream=None):
-        _check(lib.ts_step_plan_commit(self._h, C.c_uint32(flags), _stream(stream)), "ts_step_plan_commit")
+        _check(lib.ts_step_plan_commit(self._h, C.c_uint32(flags), _stream(stream, self._pool.device)), "ts_step_plan_commit")
 
     def ts_step_plan_block_bytes(self):
         return int(lib.ts_step_plan_block_bytes(self._h))

@@ -225,6 +225,9 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
         const CUtensorMap* mvn = mq + 2;
         const int32_t* pt = p.page_tables + g.pt_off;
         if (g.n_q > 0) {
+          // the Q tiles cannot land before the previous item's last S = Q K^T has read the buffer: pull them into L2 now
+          for (int i = 0; i < g.n_q; ++i)
+            for (int b = 0; b < C::kDBlocks; ++b) tma_prefetch_3d(mq, 64 * b, g.head, g.r0 + 128 * i);
           mbar_wait_long(q_empty, (q_cnt & 1) ^ 1);
           ++q_cnt;
           mbar_arrive_expect_tx(q_full, g.n_q * C::kTileBytes);

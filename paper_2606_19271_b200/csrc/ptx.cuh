@@ -99,6 +99,11 @@ __device__ __forceinline__ void tma_load_4d(void* dst, const void* map, int c0, 
       : "memory");
 }
 
+// L2 prefetch of a box (no shared-memory destination, no barrier): warms L2 for a load that cannot be issued yet.
+__device__ __forceinline__ void tma_prefetch_3d(const void* map, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global [%0, {%1, %2, %3}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
 // Multicast variants: the box lands at the same shared-memory offset of every CTA named in `mask`, and completes
 // bytes on the mbarrier at the same offset of each of them.
 __device__ __forceinline__ void tma_load_3d_mc(void* dst, const void* map, int c0, int c1, int c2, uint64_t* bar, uint16_t mask) {

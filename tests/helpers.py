@@ -65,16 +65,18 @@ class DualPool:
     MAX_ABS, REL_L2 = 2e-2, 5e-3
     NAN_BF16, HUGE_BF16 = 0x7FC0, 0x7F7F
 
-    def __init__(self, shape, free_order=None, host_pages=0, poison=NAN_BF16):
+    def __init__(self, shape, free_order=None, host_pages=0, poison=NAN_BF16, device=0):
         """Every test pool starts with its whole KV slab filled with bf16 NaN (`poison`; None: torch.empty), and every state
         check refills the pages on the free list: a result that depends on a byte the library has not written itself (a
         stale page behind a grown table, a recycled page) turns into a NaN in the output instead of passing by luck."""
         from paper_2606_19271_b200 import TurboChunkPool
         self.shape = shape
+        self.dev = f"cuda:{device}"
         self.o = make_oracle_pool(shape, free_order, host_pages if host_pages else None)
         self.g = TurboChunkPool(shape.n_layers, shape.n_heads, shape.head_dim, shape.page_tokens, shape.n_pages,
                                 shape.frame_tokens, shape.window_frames, shape.max_sessions,
-                                free_order=free_order, host_pages=host_pages, guard_bytes=1 << 20, poison=poison)
+                                free_order=free_order, host_pages=host_pages, guard_bytes=1 << 20, poison=poison,
+                                device=device)
 
     def open(self):
         a, b = self.o.open(), self.g.ts_session_open()
@@ -88,7 +90,7 @@ class DualPool:
     def append(self, layer, sids, cf, k_bits, v_bits, commit=True, dev=None):
         from paper_2606_19271_b200 import TS_COMMIT
         self.o.append(layer, sids, cf, k_bits, v_bits, commit=commit)
-        dk, dv = dev if dev is not None else (bits_to_dev(k_bits), bits_to_dev(v_bits))
+        dk, dv = dev if dev is not None else (bits_to_dev(k_bits, self.dev), bits_to_dev(v_bits, self.dev))
         self.g.ts_kv_append(layer, sids, cf, dk, dv, TS_COMMIT if commit else 0)
 
     def feed_prior(self, sid, k_layers, v_layers, frames_per_append=3):
@@ -114,11 +116,11 @@ class DualPool:
     def attention(self, layer, sids, cf, q_bits, k_bits, v_bits, scale, check=True, with_lse=True):
         import torch
         o_ref, lse_ref = oracle.chunk_attention(self.o, layer, sids, cf, q_bits, k_bits, v_bits, scale)
-        dq, dk, dv = bits_to_dev(q_bits), bits_to_dev(k_bits), bits_to_dev(v_bits)
+        dq, dk, dv = (bits_to_dev(x, self.dev) for x in (q_bits, k_bits, v_bits))
         out = torch.full_like(dq, float("nan"))
         lse = torch.full(dq.shape[:2], float("nan"), dtype=torch.float32, device=dq.device) if with_lse else None
         self.g.ts_chunk_attention(layer, sids, cf, dq, dk, dv, out, lse, float(scale))
-        torch.cuda.synchronize()
+        torch.cuda.synchronize(self.dev)
         o_gpu = out.double().cpu().numpy()
         if check:
             assert np.isfinite(o_gpu).all()
@@ -137,10 +139,10 @@ class DualPool:
         from paper_2606_19271_b200 import TS_COMMIT
         o_ref, _ = oracle.chunk_attention(self.o, layer, sids, cf, q_bits, k_bits, v_bits, scale)
         self.o.append(layer, sids, cf, k_bits, v_bits, commit=commit)
-        dq, dk, dv = dev if dev is not None else (bits_to_dev(q_bits), bits_to_dev(k_bits), bits_to_dev(v_bits))
+        dq, dk, dv = dev if dev is not None else tuple(bits_to_dev(x, self.dev) for x in (q_bits, k_bits, v_bits))
         out = torch.full_like(dq, float("nan"))
         self.g.ts_chunk_step(layer, sids, cf, dq, dk, dv, out, None, float(scale), TS_COMMIT if commit else 0)
-        torch.cuda.synchronize()
+        torch.cuda.synchronize(self.dev)
         o_gpu = out.double().cpu().numpy()
         assert np.isfinite(o_gpu).all(), "fused step: non-finite output (a masked operand read bytes the library never wrote)"
         max_abs = float(np.abs(o_gpu - o_ref).max())
@@ -165,7 +167,7 @@ class DualPool:
             if kv and io["state"] == oracle.RESIDENT:
                 for layer in (layers if layers is not None else range(self.shape.n_layers)):
                     gk, gv = self.g.ts_gather_kv(layer, sid)
-                    torch.cuda.synchronize()
+                    torch.cuda.synchronize(self.dev)
                     ok, ov = self.o.gather_kv(layer, sid)
                     assert np.array_equal(dev_to_bits(gk), ok), f"K bytes differ sid={sid} layer={layer}"
                     assert np.array_equal(dev_to_bits(gv), ov), f"V bytes differ sid={sid} layer={layer}"

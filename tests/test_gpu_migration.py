@@ -244,3 +244,37 @@ def test_migration_full_window_wan13b():
     a.check_state([sid])
     nbytes = a.g.ts_session_info(sid)["n_pages"] * a.g.page_bytes
     print(f"migrate {nbytes / 1e6:.0f} MB: {np.median(times) * 1e3:.0f} us, {2 * nbytes / np.median(times) / 1e6:.0f} GB/s read+write")
+
+
+# ---- two devices: the fetch kernel runs on the target GPU and reads the source slab through the peer mapping (NVLink) ----
+@pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs two GPUs with peer access (one-GPU boxes run the same "
+                    "kernel with both pools on one device: every other test of this file)")
+def test_migration_between_two_devices():
+    """Pools on devices 0 and 1 of this process; a session migrates 0 -> 1, is served there, migrates back 1 -> 0 and is
+    served again: ids, page tables, free lists, logical KV bytes against the oracle on both devices, attention on the
+    target within tolerance."""
+    if not (torch.cuda.can_device_access_peer(0, 1) and torch.cuda.can_device_access_peer(1, 0)):
+        pytest.skip("no peer access between devices 0 and 1")
+    sh = shape_of(n_heads=3, head_dim=128, page_tokens=64, frame_tokens=130, window_frames=6, n_pages=48, n_layers=2)
+    rng = np.random.default_rng(77)
+    pools = [DualPool(sh, rng.permutation(sh.n_pages), device=d) for d in (0, 1)]
+    T = sh.frame_tokens
+    sid = pools[0].open()
+    other = [pools[0].open(), pools[1].open()]                 # bystanders on both devices
+    add_frames(pools[0], sid, rng, 5)
+    add_frames(pools[0], other[0], rng, 2)
+    add_frames(pools[1], other[1], rng, 3)
+    where = 0
+    for hop in range(4):                                       # 0 -> 1 -> 0 -> 1 -> 0, the window rolling on the way
+        src, dst = pools[where], pools[where ^ 1]
+        sid = migrate(src, sid, dst)
+        where ^= 1
+        dst.check_state([sid, other[where]])
+        src.check_state([other[where ^ 1]])
+        with torch.cuda.device(where):
+            for layer in range(sh.n_layers):
+                q, k, v = (draw(rng, 3 * T, sh) for _ in range(3))
+                dst.fused_step(layer, [sid, other[where]], [2, 1], q, k, v, scale_of(sh), commit=(layer == sh.n_layers - 1))
+        dst.check_state([sid, other[where]])
+    for p in pools:
+        p.g.close()
