@@ -127,6 +127,21 @@ struct Staging {      // pinned (mapped) host + device buffer pair for per-call 
 
 using namespace tc;
 
+// The KV append of a fused chunk step, prepared on the host (pages already allocated) and carried out by the idle
+// warps of the attention kernel.
+struct FusedAppend {
+  std::vector<CopySess> cs;            // pt_off is filled in from the attention schedule (same packed page tables)
+  uint64_t wait_side = 0, wait_compute = 0;
+  int total_rows = 0;
+  std::vector<int32_t> popped;         // page ids taken from the free list, in pop order (rolled back on failure)
+  void reset() {
+    cs.clear();
+    popped.clear();
+    wait_side = wait_compute = 0;
+    total_rows = 0;
+  }
+};
+
 struct ts_pool {
   ts_pool_config cfg;
   int log2_B = 0;
@@ -161,6 +176,8 @@ struct ts_pool {
   std::vector<int32_t> scratch_need;       // per-session page demand of the call in progress
   std::vector<int64_t> scratch_key;        // schedule key of the call in progress
   std::vector<uint8_t*> retired;           // outgrown staging buffers, freed with the pool (never under running work)
+  FusedAppend scratch_fused_obj;            // descriptors of the fused append of the call in progress
+  FusedAppend* scratch_fused = &scratch_fused_obj;
   // attention schedule of the last batch (a1), reused while the batch and its sessions' page tables are unchanged:
   // every layer and denoising pass of one chunk step then pays the scheduler once
   uint64_t ver_seq = 0;                    // source of Session::ver values (never repeats, also across reopen)
@@ -821,15 +838,6 @@ static int64_t page_demand(ts_pool* pool, int32_t n, const int32_t* sids, const 
   return total;
 }
 
-// The KV append of a fused chunk step, prepared on the host (pages already allocated) and carried out by the idle
-// warps of the attention kernel.
-struct FusedAppend {
-  std::vector<CopySess> cs;            // pt_off is filled in from the attention schedule (same packed page tables)
-  uint64_t wait_side = 0, wait_compute = 0;
-  int total_rows = 0;
-  std::vector<int32_t> popped;         // page ids taken from the free list, in pop order (rolled back on failure)
-};
-
 // Grows the page tables of the batch by pool->scratch_need (popping from the front of the free list, sessions in `sids`
 // order) and describes the append of the chunks that follows.  The caller has checked the demand against the free list.
 static void grow_for_append(ts_pool* pool, int32_t n, const int32_t* sids, const int32_t* chunk_frames, FusedAppend* fa) {
@@ -967,17 +975,10 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, c
   const int T = c.frame_tokens, B = c.page_tokens;
 
   // demand check first: all-or-nothing (O2)
-  std::vector<int> need(n);
-  int64_t need_total = 0;
+  const int64_t need_total = page_demand(pool, n, sids, chunk_frames);
+  const std::vector<int32_t>& need = pool->scratch_need;
   size_t n_pt_total = 0;
-  for (int b = 0; b < n; ++b) {
-    const Session& s = pool->sess[sids[b]];
-    const int64_t end = (int64_t)s.o + (int64_t)s.P * T + (int64_t)chunk_frames[b] * T;
-    need[b] = (int)((end + B - 1) / B) - (int)s.pt.size();
-    if (need[b] < 0) need[b] = 0;
-    need_total += need[b];
-    n_pt_total += s.pt.size() + need[b];
-  }
+  for (int b = 0; b < n; ++b) n_pt_total += pool->sess[sids[b]].pt.size() + need[b];
   if (need_total > (int64_t)pool->free_q.size()) return TS_ERR_NO_PAGES;
 
   const size_t off_sess = 0;
@@ -1063,7 +1064,8 @@ int ts_chunk_step(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, 
   // grow the page tables first: the attention schedule is then built from the grown tables (the attention itself only
   // reads [x_begin, x_end), R5) and its packed page-table array also serves the append, which the idle warps of the
   // attention kernel carry out - it is HBM-bound, the attention is not, so it costs the step nothing there
-  FusedAppend fa;
+  FusedAppend& fa = *pool->scratch_fused;   // (the vectors keep their capacity from call to call)
+  fa.reset();
   grow_for_append(pool, n, sids, chunk_frames, &fa);
   uint64_t seq = 0;
   rc = attention_impl(pool, layer, n, sids, chunk_frames, q, k, v, out, lse, scale, cuda_stream, &fa, &seq);
@@ -1205,7 +1207,8 @@ int ts_step_plan_prepare(ts_step_plan* plan, void* cuda_stream) {
     TS_CUDA(cudaEventSynchronize(plan->h_ev[slot]));
     plan->h_busy[slot] = false;
   }
-  FusedAppend fa;
+  FusedAppend& fa = *pool->scratch_fused;
+  fa.reset();
   grow_for_append(pool, n, sids, cf, &fa);
   build_schedule(pool, n, sids, cf);
   if (pool->sched_pt.size() > plan->max_pt || pool->sched_items.size() > plan->max_items) {   // cannot happen: bounds above

@@ -538,6 +538,81 @@ def test_latency_model_sweep_small():
     assert rows[1][0] > rows[0][0]          # four sessions take longer than one
 
 
+def test_latency_model_is_linear_in_n_at_full_size():
+    """l_hat(n) on the Wan-1.3B shape at the full 21-frame window (the one quantity the controllers take from the
+    runtime): attention time per layer is linear in the number of co-located sessions - every n within +-10 % of the
+    per-session time fitted through the sweep - and the values are in the band the B200 can produce at all (0.55-1.0 ms
+    per session-layer = 1100-1700 TFLOP/s ... a plausibility band, not a performance claim)."""
+    from paper_2606_19271_b200 import latency_model
+    ns = (2, 4, 8, 16)
+    ms = [latency_model.measure(n, 18, 12, 128, 1560, 21, 256, reps=5)[0] for n in ns]
+    per = float(np.sum(np.array(ms) * np.array(ns)) / np.sum(np.array(ns) ** 2))        # least squares through the origin
+    for n, t in zip(ns, ms):
+        assert abs(t / (per * n) - 1.0) <= 0.10, (n, t, per)
+    assert 0.55 <= per <= 1.0, per
+
+
+def test_resumed_session_is_served_by_the_next_step_without_a_host_wait():
+    """PAPER.md:76 (iii) "restored ... before chunk generation resumes": a full-window session is resumed while the other
+    sessions' step is being enqueued and is in the NEXT step's batch.  The host never waits for the copy (both calls return in
+    a small fraction of the 4 ms the 201 MB copy takes; the step's launch waits for the resume's event on the stream), and the
+    output of the step that serves it matches the oracle."""
+    import time
+    from synth.draw import draw_bits_torch
+    from paper_2606_19271_b200 import TS_COMMIT
+    shape = shape_of(n_heads=12, head_dim=128, frame_tokens=1560, window_frames=21, page_tokens=256, n_pages=3 * 140,
+                     max_sessions=4)
+    rng = np.random.default_rng(60)
+    dp = DualPool(shape, rng.permutation(shape.n_pages), host_pages=140)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(60)
+    T, H, D = shape.frame_tokens, shape.n_heads, shape.head_dim
+    a, b = dp.open(), dp.open()
+    for _ in range(6):                                           # both at the full window (18 prior frames)
+        for sid in (a, b):
+            dk, dv = draw_bits_torch(gen, 3 * T, H, D, "cuda"), draw_bits_torch(gen, 3 * T, H, D, "cuda")
+            dp.append(0, [sid], [3], dev_to_bits(dk), dev_to_bits(dv), dev=(dk, dv))
+    dp.suspend(b)
+    dp.g.ts_offload_sync()
+    qa, ka, va = (draw_bits_torch(gen, 3 * T, H, D, "cuda") for _ in range(3))
+    qb, kb, vb = (draw_bits_torch(gen, 3 * T, H, D, "cuda") for _ in range(3))
+    q2, k2, v2 = (torch.cat([x, y]) for x, y in ((qa, qb), (ka, kb), (va, vb)))
+    out1, out2 = torch.empty_like(qa), torch.full_like(q2, float("nan"))
+    scale = float(scale_of(shape))
+    dp.o.resume(b)
+    torch.cuda.synchronize()
+    side = dp.g.side_stream
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    e0.record(side)
+    dp.g.ts_session_resume(b)                                    # step t: the resume of b is enqueued ...
+    e1.record(side)
+    dp.g.ts_chunk_step(0, [a], [3], qa, ka, va, out1, None, scale, 0)          # ... while a is served
+    dp.g.ts_chunk_step(0, [a, b], [3, 3], q2, k2, v2, out2, None, scale, 0)    # step t + 1 serves b
+    host_ms = (time.perf_counter() - t0) * 1e3
+    torch.cuda.synchronize()
+    copy_ms = e0.elapsed_time(e1)
+    assert copy_ms > 2.0, copy_ms                                # 201 MB over the host link
+    assert host_ms < 0.5 * copy_ms, (host_ms, copy_ms)           # the host was back long before the copy had finished
+    rs = np.random.default_rng(61)
+    C = 3 * T
+    o_gpu = out2.double().cpu().numpy()
+    assert np.isfinite(o_gpu).all()
+    errs, refs = [], []
+    for i, (sid, (qq, kk, vv)) in enumerate(((a, (qa, ka, va)), (b, (qb, kb, vb)))):
+        rows = np.unique(np.concatenate([rs.integers(0, C, size=12), [0, T, C - 1]]))
+        h = int(rs.integers(0, H))
+        o_ref, _ = oracle.attention_rows(dp.o, 0, sid, 3, dev_to_bits(qq), dev_to_bits(kk), dev_to_bits(vv), scale_of(shape), h, rows)
+        errs.append(o_gpu[i * C + rows, h] - o_ref)
+        refs.append(o_ref)
+    err, ref = np.concatenate(errs), np.concatenate(refs)
+    assert np.abs(err).max() <= 2e-2 and np.linalg.norm(err) / np.linalg.norm(ref) <= 5e-3
+    dp.o.append(0, [a], [3], dev_to_bits(ka), dev_to_bits(va), commit=False)       # the two uncommitted appends of the steps
+    dp.o.append(0, [a, b], [3, 3], dev_to_bits(k2), dev_to_bits(v2), commit=False)
+    dp.check_state([a, b], kv=False)
+    dp.g.close()
+
+
 # ---- ts_chunk_step_host: the host-buffer entry point (H2D, attention, append, D2H), two pipelined steps ------------
 def test_chunk_step_host_two_steps():
     from paper_2606_19271_b200 import TS_COMMIT
