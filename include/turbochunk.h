@@ -133,7 +133,8 @@ int ts_session_close(ts_pool* pool, int32_t sid);
  *     U the chunk's own tokens of frames <= f  (frame-block-causal, R1).
  * bf16 operands, fp32 accumulation and fp32 online softmax, bf16 output (R3, R4).
  *   q, k, v, out : device bf16 [sum_b C_b][H][D], sessions concatenated in sids order, no padding (R15);
- *                  C_b = chunk_frames[b] * T.  16-byte aligned.
+ *                  C_b = chunk_frames[b] * T.  q, k, v 16-byte aligned, out 32-byte aligned (it is written with 256-bit
+ *                  stores, one full 32-byte sector per lane).
  *   lse          : device fp32 [sum_b C_b][H] natural-log logsumexp of the scaled logits, or NULL.
  *   scale        : softmax scale (R2).
  *   cuda_stream  : cudaStream_t of the caller (NULL = legacy default stream).

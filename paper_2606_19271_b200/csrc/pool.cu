@@ -893,7 +893,7 @@ static int attention_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t
   if (rc != TS_OK) return rc;
   if (n == 0) return TS_OK;
   if (q == nullptr || k == nullptr || v == nullptr || out == nullptr) return TS_ERR_INVALID;
-  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) != 0) return TS_ERR_INVALID;
+  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v) & 15) != 0 || ((uintptr_t)out & 31) != 0) return TS_ERR_INVALID;
   if (!(scale > 0.0f) || !std::isfinite(scale)) return TS_ERR_INVALID;
   const ts_pool_config& c = pool->cfg;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
@@ -1056,7 +1056,7 @@ int ts_chunk_step(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, 
   if (rc != TS_OK) return rc;
   if (n == 0) return TS_OK;
   if (q == nullptr || k == nullptr || v == nullptr || out == nullptr) return TS_ERR_INVALID;
-  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) != 0) return TS_ERR_INVALID;
+  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v) & 15) != 0 || ((uintptr_t)out & 31) != 0) return TS_ERR_INVALID;
   if (!(scale > 0.0f) || !std::isfinite(scale)) return TS_ERR_INVALID;
   if ((flags & ~(uint32_t)TS_COMMIT) != 0) return TS_ERR_INVALID;
   // page demand of the append, before anything changes or is enqueued (all-or-nothing, O2)
@@ -1176,7 +1176,7 @@ int ts_step_plan_create(ts_pool* pool, int32_t n, const int32_t* sids, const int
 int ts_step_plan_bind(ts_step_plan* plan, int32_t slot, const void* q, const void* k, const void* v, void* out, float* lse) {
   if (plan == nullptr || slot < 0 || slot >= plan->n_slots) return TS_ERR_INVALID;
   if (q == nullptr || k == nullptr || v == nullptr || out == nullptr) return TS_ERR_INVALID;
-  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15) != 0) return TS_ERR_INVALID;
+  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v) & 15) != 0 || ((uintptr_t)out & 31) != 0) return TS_ERR_INVALID;
   if (plan->prepared) return TS_ERR_STATE;   // the maps travel with the prepare upload
   if (!encode_session_maps(plan->pool, plan->maps.data() + (size_t)slot * plan->n * 3, plan->n, plan->cf.data(), q, k, v))
     return TS_ERR_CUDA;

@@ -808,3 +808,27 @@ def test_lazy_rescale_and_outliers(pattern, page_tokens):
     q2, k2, v2 = (draw(rng, 3 * T, shape) for _ in range(3))
     dp.attention(0, [other, sid], [3, c], np.concatenate([q2, qb]), np.concatenate([k2, kb[Lp:]]),
                  np.concatenate([v2, vb[Lp:]]), scale_of(shape))
+
+
+def test_output_alignment_is_checked():
+    """`out` is written with 256-bit stores: a pointer that is 16- but not 32-byte aligned is TS_ERR_INVALID, not a fault."""
+    import paper_2606_19271_b200 as tc
+    shape = shape_of(n_heads=1, head_dim=64, frame_tokens=16, window_frames=0, page_tokens=16, n_pages=8)
+    dp = DualPool(shape)
+    sid = dp.open()
+    rng = np.random.default_rng(1)
+    q, k, v = (bits_to_dev(draw(rng, 16, shape)) for _ in range(3))
+    raw = torch.empty(16 * 64 + 16, dtype=torch.bfloat16, device="cuda")
+    assert raw.data_ptr() % 32 == 0
+    bad = raw[8:8 + 16 * 64].view(16, 1, 64)                     # 16 bytes past a 32-byte boundary
+    for call in (lambda o: dp.g.ts_chunk_attention(0, [sid], [1], q, k, v, o, None, 0.125),
+                 lambda o: dp.g.ts_chunk_step(0, [sid], [1], q, k, v, o, None, 0.125, tc.TS_COMMIT)):
+        with pytest.raises(tc.TurboChunkError) as e:
+            call(bad)
+        assert e.value.code == tc.TS_ERR_INVALID
+    dp.check_state([sid])
+    good = raw[:16 * 64].view(16, 1, 64)
+    dp.g.ts_chunk_attention(0, [sid], [1], q, k, v, good, None, 0.125)
+    torch.cuda.synchronize()
+    assert torch.isfinite(good.float()).all()
+    dp.g.close()
