@@ -281,7 +281,8 @@ int ts_pool_free_list(ts_pool* pool, int32_t* out, int32_t cap, int32_t* n_out);
 int ts_pool_stats(ts_pool* pool, ts_pool_stats_t* out);
 /* The side stream in use (cudaStream_t), for timing offload with events. */
 void* ts_pool_side_stream(ts_pool* pool);
-/* Number of kernels the library has launched on this pool since creation (bench.py's gpu_launches). */
+/* Number of kernels the library has launched on this pool since creation, descriptor-upload kernels included
+ * (bench.py's gpu_launches). */
 int64_t ts_pool_launch_count(ts_pool* pool);
 
 /* Number of times the ragged batch scheduler (a1) had to build a schedule (the rest were reuses of the cached one). */

@@ -237,6 +237,7 @@ static int upload_staging(ts_pool* pool, Staging* st, size_t bytes, cudaStream_t
     TS_CUDA(cudaStreamCreateWithPriority(&pool->up_s, cudaStreamNonBlocking, hi));
   }
   TS_CUDA(launch_upload(st->h_dev, st->d, align_up(bytes, 16), pool->up_s));
+  ++pool->launches;
   TS_CUDA(cudaEventRecord(st->ev_up, pool->up_s));
   TS_CUDA(cudaStreamWaitEvent(consumer, st->ev_up, 0));
   return TS_OK;
@@ -1225,6 +1226,7 @@ int ts_step_plan_prepare(ts_step_plan* plan, void* cuda_stream) {
   if (e == cudaSuccess) e = pool->tl_compute.wait(stream, fa.wait_compute);
   // the block is rewritten in stream order: after the previous step's launches, before this step's
   if (e == cudaSuccess) e = launch_upload(plan->h_dev[slot], plan->d, align_up(plan->L.bytes, 16), stream);
+  ++pool->launches;
   if (e == cudaSuccess) e = cudaEventRecord(plan->h_ev[slot], stream);
   if (!cuda_ok(e, "ts_step_plan_prepare")) {
     ungrow(pool, n, sids, fa);
@@ -1466,6 +1468,7 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
     TS_CUDA_UNDO(src->tl_side.wait(dst->side, s.side_seq));
     TS_CUDA_UNDO(dst->tl_compute.wait(dst->side, wait_compute));
     TS_CUDA_UNDO(launch_upload(st->h_dev, st->d, align_up(n * 8, 16), dst->side));   // not a DMA copy: see upload_staging
+    ++dst->launches;
     PullParams p;
     p.src_slab = src->slab;
     p.dst_slab = dst->slab;

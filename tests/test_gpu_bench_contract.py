@@ -31,7 +31,7 @@ def test_bench_line_contract():
     assert r["bound"] == "tensor" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-3
     assert r["traffic"] is None or r["traffic"] > 0
     assert 0.3 < r["frac"] < 1.0 and d["value"] > 500
-    assert d["gpu_launches"] == 5                                   # one fused launch per timed step + one committed step
+    assert d["gpu_launches"] == 2 * 5                               # (descriptor upload + fused launch) per timed step + one committed step
     assert r["ms_per_launch"] <= d["ms_per_step"]                   # the roofline comes from the timed loop itself
     assert d["step"]["sched_builds_in_timed_loop"] >= 2             # a1 is inside timed steps, not only the cached reuse
     assert 1000 < d["clocks"]["sm_mhz_in_kernel"] <= d["clocks"]["sm_max_mhz"] + 50

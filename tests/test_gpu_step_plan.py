@@ -105,7 +105,7 @@ def test_multilayer_step_plan_matches_oracle(page_tokens, use_graph):
         dp.check_state(sids)
     if use_graph:
         # the capture recorded NL * passes launches once; the four replays launched nothing through the host path
-        assert dp.g.ts_pool_launch_count() - launches0 < 5 * NL * passes + 5 * NL * 3   # (check_state's gathers count too)
+        assert dp.g.ts_pool_launch_count() - launches0 < 5 * NL * passes + 5 * (NL * 3 * 2 + 1)   # (check_state's gathers and uploads count too)
     # a suspended session in the batch: prepare fails with TS_ERR_STATE and changes nothing
     dp.suspend(sids[1])
     with pytest.raises(tc.TurboChunkError) as e:
