@@ -54,6 +54,15 @@ def test_invalid_config_rejected_before_cuda(tc):
     assert tc.lib.ts_pool_create(C.byref(cfg), C.byref(h)) == tc.TS_ERR_INVALID
     assert tc.lib.ts_pool_create(None, C.byref(h)) == tc.TS_ERR_INVALID
     assert tc.lib.ts_session_open(None, None) == tc.TS_ERR_INVALID
+    # the step-plan calls reject null handles before touching CUDA
+    assert tc.lib.ts_step_plan_create(None, 1, None, None, 1, C.byref(h)) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_step_plan_bind(None, 0, None, None, None, None, None) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_step_plan_prepare(None, None) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_step_plan_run(None, 0, 0, C.c_float(1.0), 0, None) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_step_plan_commit(None, 0, None) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_step_plan_destroy(None) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_step_plan_block_bytes(None) == 0
+    assert tc.lib.ts_pool_clock_probe(None, None) == tc.TS_ERR_INVALID and tc.lib.ts_pool_sched_builds(None) == 0
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
