@@ -150,6 +150,33 @@ class DualPool:
         assert max_abs <= self.MAX_ABS and rl2 <= self.REL_L2, (max_abs, rl2)
         return o_gpu, o_ref
 
+    def plan_step(self, sids, cf, q_bits, k_bits, v_bits, scale, n_layers, passes=1):
+        """A whole multi-layer chunk step through ts_step_plan_* (one buffer set, the same tensors on every layer; attention-only
+        launches for all passes but the last, which also appends; TS_COMMIT) against the oracle's attention per layer, appends on
+        every layer and the commit on the last."""
+        import torch
+        from paper_2606_19271_b200 import TS_COMMIT, TS_RUN_APPEND
+        refs = [oracle.chunk_attention(self.o, l, sids, cf, q_bits, k_bits, v_bits, scale)[0] for l in range(n_layers)]
+        for l in range(n_layers):
+            self.o.append(l, sids, cf, k_bits, v_bits, commit=(l == n_layers - 1))
+        dq, dk, dv = (bits_to_dev(x, self.dev) for x in (q_bits, k_bits, v_bits))
+        outs = [torch.full_like(dq, float("nan")) for _ in range(n_layers)]
+        plan = self.g.ts_step_plan_create(sids, cf, n_slots=n_layers)
+        for l in range(n_layers):
+            plan.ts_step_plan_bind(l, dq, dk, dv, outs[l], None)
+        plan.ts_step_plan_prepare()
+        for p in range(passes):
+            for l in range(n_layers):
+                plan.ts_step_plan_run(l, l, float(scale), TS_RUN_APPEND if p == passes - 1 else 0)
+        plan.ts_step_plan_commit(TS_COMMIT)
+        torch.cuda.synchronize(self.dev)
+        plan.close()
+        for l in range(n_layers):
+            o_gpu = outs[l].double().cpu().numpy()
+            assert np.isfinite(o_gpu).all(), "step plan: non-finite output"
+            max_abs, rl2 = float(np.abs(o_gpu - refs[l]).max()), rel_l2(o_gpu, refs[l])
+            assert max_abs <= self.MAX_ABS and rl2 <= self.REL_L2, (l, max_abs, rl2)
+
     def check_state(self, sids, layers=None, kv=True):
         import torch
         # compute-sanitizer is closed on the GPU pool: 1 MiB guard bands around the slab and the pinned arena stand in for it

@@ -14,7 +14,7 @@ from helpers import DualPool, bits_to_dev
 pytestmark = pytest.mark.gpu
 
 
-def run_case(seed, large):
+def run_case(seed, large, use_plan=False):
     import paper_2606_19271_b200 as tc
     rng = np.random.default_rng(1000 + seed)
     if large:
@@ -44,7 +44,9 @@ def run_case(seed, large):
     layer = int(rng.integers(0, NL))
     dp.attention(layer, sids, cf, q, k, v, scale)
     dev = (bits_to_dev(q), bits_to_dev(k), bits_to_dev(v))
-    for l in range(NL):
+    if use_plan:        # the same step through the capture-safe plan calls (one prepare, NL x 2 launches, one commit)
+        dp.plan_step(sids, cf, q, k, v, scale, NL, passes=2)
+    for l in range(0 if use_plan else NL):
         # layer l > 0 runs on page tables that layer 0's uncommitted append has already grown: the slab is NaN-poisoned
         # (DualPool), so a gather that strays onto a not-yet-written page shows up in `out`, which is compared here
         dp.fused_step(l, sids, cf, q, k, v, scale, commit=(l == NL - 1), dev=dev)
@@ -62,3 +64,8 @@ def test_small_shapes(seed):
 @pytest.mark.parametrize("seed", range(200, 208))
 def test_larger_shapes(seed):
     run_case(seed, large=True)
+
+
+@pytest.mark.parametrize("seed", range(400, 412))
+def test_shapes_through_step_plan(seed):
+    run_case(seed, large=(seed % 3 == 0), use_plan=True)
