@@ -220,6 +220,7 @@ int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
  * (attention, append, step, suspend, close, migrate, another plan) returns TS_ERR_STATE.  Launches of one plan must not
  * overlap in time (one stream, or ordered streams): they share the plan's work-item cursor, which each launch rearms
  * for the next.  A graph captured between a prepare and a commit may be replayed after any later prepare of the same plan.
+ * A plan points into its pool: destroy it before ts_pool_destroy.
  * Errors: create: as ts_chunk_attention's batch checks, TS_ERR_CUDA; bind: TS_ERR_INVALID (slot, null or misaligned
  * pointer), TS_ERR_STATE (plan prepared); run: TS_ERR_STATE (not prepared, slot not bound), TS_ERR_INVALID.
  */

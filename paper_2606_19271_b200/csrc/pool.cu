@@ -1225,8 +1225,10 @@ int ts_step_plan_prepare(ts_step_plan* plan, void* cuda_stream) {
   if (e == cudaSuccess) e = pool->tl_side.wait(stream, fa.wait_side);
   if (e == cudaSuccess) e = pool->tl_compute.wait(stream, fa.wait_compute);
   // the block is rewritten in stream order: after the previous step's launches, before this step's
-  if (e == cudaSuccess) e = launch_upload(plan->h_dev[slot], plan->d, align_up(plan->L.bytes, 16), stream);
-  ++pool->launches;
+  if (e == cudaSuccess) {
+    e = launch_upload(plan->h_dev[slot], plan->d, align_up(plan->L.bytes, 16), stream);
+    ++pool->launches;
+  }
   if (e == cudaSuccess) e = cudaEventRecord(plan->h_ev[slot], stream);
   if (!cuda_ok(e, "ts_step_plan_prepare")) {
     ungrow(pool, n, sids, fa);
