@@ -782,7 +782,7 @@ def measure_overlap(wl, out, reps=12):
                     "and the steps it hides behind run `step_slowdown` slower"}
 
 
-def measure_latency_model(ns=(1, 2, 4, 5, 6, 8, 16, 32), layers=30, passes=4, slo_ms=670.0):
+def measure_latency_model(ns=(1, 2, 4, 5, 6, 7, 8, 16, 32), layers=30, passes=4, slo_ms=670.0):
     """l_hat(n): per-layer attention + append time against the number of co-located full-window sessions,
     and the largest n whose 30-layer x 4-pass lower bound meets the 670 ms SLO."""
     from paper_2606_19271_b200.latency_model import measure

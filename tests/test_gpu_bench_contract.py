@@ -40,7 +40,7 @@ def test_bench_line_contract():
     o = d["overlap"]
     assert 0.9 * o["step_alone_ms"] <= o["step_with_offload_ms"] <= 1.5 * o["step_alone_ms"] and o["resume_h2d_gbs_under_load"] > 10
     lm = d["latency_model"]
-    assert [x["n"] for x in lm["l_hat"]] == [1, 2, 4, 5, 6, 8, 16, 32] and lm["largest_n_under_slo"] >= 1
+    assert [x["n"] for x in lm["l_hat"]] == [1, 2, 4, 5, 6, 7, 8, 16, 32] and lm["largest_n_under_slo"] >= 1
     cfgs = d["configs"]
     assert set(cfgs) == {"configs[1]", "configs[3]", "configs[4]"}
     assert cfgs["configs[3]"]["chunk_step_graph"]["graph_launches"] == 1
