@@ -182,7 +182,10 @@ int ts_chunk_step(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /
  *       and stay unchanged until `cuda_stream` has passed the call.  That is what lets the input copy of one call
  *       run under the attention and the output copy of the previous one (two staging sets).
  *   out_host : host bf16, same shape; complete once `cuda_stream` has passed the call (stream order).
- * Staging grows on demand (cudaMalloc, with a device synchronisation) and is reused.  Errors as the two calls.
+ * Staging grows on demand (cudaMalloc; an outgrown buffer is kept until the pool is destroyed, nothing is waited for) and is
+ * reused.  q_host, k_host, v_host packed behind one another ([3][sum C][H][D], tensor size a multiple of 1024 bytes) are copied
+ * in ONE transfer.  Runs the fused ts_chunk_step (one launch).  All-or-nothing: arguments, states and the page demand are
+ * checked before a single copy is enqueued (TS_ERR_NO_PAGES leaves out_host untouched).
  */
 int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
                        const void* q_host, const void* k_host, const void* v_host, void* out_host,
@@ -203,7 +206,7 @@ int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
  *     ts_step_plan_prepare(plan, stream)      NOT capturable.  Validates as ts_chunk_step (TS_ERR_STATE, TS_ERR_NO_PAGES;
  *                                             all-or-nothing), grows the page tables for the step's append, builds the
  *                                             schedule (a1) and writes it into the plan's device block in stream order
- *                                             (one H2D of the whole block); enqueues the stream-side waits (pending
+ *                                             (one small copy kernel reading mapped pinned memory); enqueues the stream-side waits (pending
  *                                             resumes, copies out of recycled pages).  The block's address, the grid
  *                                             and every kernel argument are the same for every prepare of a plan.
  *     ts_step_plan_run(plan, layer, slot, scale, run_flags, stream)

@@ -119,7 +119,7 @@ struct Staging {      // pinned (mapped) host + device buffer pair for per-call 
   uint8_t* d = nullptr;
   size_t cap = 0;
   cudaEvent_t ev = nullptr;      // recorded on the consumer's stream after the kernel that reads `d`
-  cudaEvent_t ev_up = nullptr;   // recorded on the pool's upload stream after the H2D of the block
+  cudaEvent_t ev_up = nullptr;   // recorded on the pool's upload stream after the upload kernel of the block
   bool in_flight = false;
 };
 
