@@ -168,6 +168,11 @@ int ts_kv_append(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*
  * HBM-bound while the attention is not, so it is carried out INSIDE the attention launch, by the two warps of every
  * CTA that have no other role: one kernel, and the step takes what the attention takes.
  * Arguments as in the two calls.  All-or-nothing: arguments and page demand are checked before anything changes.
+ * PAPER.md:76 (iii): when some sessions of the batch still have a resume in flight on the side stream and others do not, the
+ * call (like ts_chunk_attention) runs as TWO launches - the ready sessions first, the resuming ones behind their copy events -
+ * so that the ready sessions' attention hides the copies instead of following them; results are those of one launch.  (A
+ * CUDA failure between the two leaves the first group committed and the second group's tables grown, as after an
+ * uncommitted append.)
  */
 int ts_chunk_step(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*host*/,
                   const int32_t* chunk_frames /*host*/, const void* q, const void* k, const void* v, void* out,
@@ -291,6 +296,9 @@ int64_t ts_pool_launch_count(ts_pool* pool);
 
 /* Number of times the ragged batch scheduler (a1) had to build a schedule (the rest were reuses of the cached one). */
 int64_t ts_pool_sched_builds(ts_pool* pool);
+/* Number of attention / step calls that ran as two launches because some of their sessions still had a resume in flight
+ * (see ts_chunk_step). */
+int64_t ts_pool_split_batches(ts_pool* pool);
 /* Measurement aid: while `device_u64x2` (device, 8-byte aligned, caller-zeroed) is set, CTA 0 of every attention
  * launch (captured launches: those recorded while it was set) adds the SM cycles and the nanoseconds it ran for to
  * [0] and [1]; [0] / [1] is the SM clock in GHz under the kernel itself, which a host-side sampler cannot see.

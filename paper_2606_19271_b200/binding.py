@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = [
     "ts_pool_page_bytes", "ts_pool_slab_bytes", "ts_pool_create", "ts_pool_destroy", "ts_session_open",
     "ts_session_close", "ts_chunk_attention", "ts_kv_append", "ts_chunk_step", "ts_chunk_step_host", "ts_session_suspend",
     "ts_session_resume", "ts_session_migrate", "ts_offload_sync", "ts_session_info", "ts_session_page_table", "ts_gather_kv",
-    "ts_pool_free_list", "ts_pool_stats", "ts_pool_side_stream", "ts_pool_launch_count", "ts_pool_sched_builds",
+    "ts_pool_free_list", "ts_pool_stats", "ts_pool_side_stream", "ts_pool_launch_count", "ts_pool_sched_builds", "ts_pool_split_batches",
     "ts_pool_clock_probe", "ts_strerror",
     "ts_last_cuda_error", "ts_version",
     "ts_step_plan_create", "ts_step_plan_bind", "ts_step_plan_prepare", "ts_step_plan_run", "ts_step_plan_commit",
@@ -97,6 +97,8 @@ def _load():
     L.ts_pool_sched_builds.restype = C.c_int64
     L.ts_pool_sched_builds.argtypes = [P]
     L.ts_pool_clock_probe.argtypes = [P, P]
+    L.ts_pool_split_batches.restype = C.c_int64
+    L.ts_pool_split_batches.argtypes = [P]
     L.ts_step_plan_create.argtypes = [P, C.c_int32, I32P, I32P, C.c_int32, C.POINTER(P)]
     L.ts_step_plan_bind.argtypes = [P, C.c_int32, P, P, P, P, P]
     L.ts_step_plan_prepare.argtypes = [P, P]
@@ -327,6 +329,9 @@ class TurboChunkPool:
 
     def ts_pool_sched_builds(self):
         return int(lib.ts_pool_sched_builds(self._h))
+
+    def ts_pool_split_batches(self):
+        return int(lib.ts_pool_split_batches(self._h))
 
     def ts_pool_clock_probe(self, buf):
         """buf: torch int64[2] on the pool's device (zeroed by the caller), or None to switch the probe off."""

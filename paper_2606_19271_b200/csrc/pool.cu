@@ -175,6 +175,9 @@ struct ts_pool {
   std::vector<int32_t> scratch_mark;       // duplicate detection
   std::vector<int32_t> scratch_need;       // per-session page demand of the call in progress
   std::vector<int64_t> scratch_key;        // schedule key of the call in progress
+  std::vector<int32_t> scratch_pending, scratch_sub_sids, scratch_sub_cf, scratch_sub_off;   // run_batch(): groups of a split batch
+  std::vector<tc::CopySess> scratch_sub_cs;
+  int64_t split_batches = 0;               // batches run as two launches (ready sessions first, resuming ones behind their copies)
   std::vector<uint8_t*> retired;           // outgrown staging buffers, freed with the pool (never under running work)
   FusedAppend scratch_fused_obj;            // descriptors of the fused append of the call in progress
   FusedAppend* scratch_fused = &scratch_fused_obj;
@@ -467,6 +470,9 @@ int ts_pool_create(const ts_pool_config* cfg, ts_pool** out) {
     if (!encode_map(&pool->map_k[l], base, 4, dims, strides, box)) return fail(TS_ERR_CUDA);
     if (!encode_map(&pool->map_v[l], base + pool->kv_bytes, 4, dims, strides, box)) return fail(TS_ERR_CUDA);
   }
+  // load the attention kernel's module now (cudaFuncSetAttribute does): with lazy module loading the FIRST launch would do it,
+  // and loading allocates device memory, which waits for every copy in flight - a resume on the side stream, for one
+  if (!cuda_ok(attention_configure(cfg->head_dim), "cudaFuncSetAttribute(attention)")) return fail(TS_ERR_CUDA);
   *out = pool;
   return TS_OK;
 }
@@ -551,6 +557,7 @@ int ts_pool_stats(ts_pool* pool, ts_pool_stats_t* out) {
 
 void* ts_pool_side_stream(ts_pool* pool) { return pool ? (void*)pool->side : nullptr; }
 int64_t ts_pool_sched_builds(ts_pool* pool) { return pool ? pool->sched_builds : 0; }
+int64_t ts_pool_split_batches(ts_pool* pool) { return pool ? pool->split_batches : 0; }
 int ts_pool_clock_probe(ts_pool* pool, void* device_u64x2) {
   if (pool == nullptr || ((uintptr_t)device_u64x2 & 7) != 0) return TS_ERR_INVALID;
   pool->clock_probe = (unsigned long long*)device_u64x2;
@@ -562,7 +569,10 @@ int64_t ts_pool_launch_count(ts_pool* pool) { return pool ? pool->launches : 0; 
 // ---- a1: collect + coalesce.  The schedule (session descriptors, packed page tables, cluster work items) depends only
 // on the batch and on its sessions' page-table state, so it is built once and reused by every later call with the same
 // key - all layers and denoising passes of a chunk step.  Result in pool->sched_*.
-static void build_schedule(ts_pool* pool, int32_t n, const int32_t* sids, const int32_t* chunk_frames) {
+// `q_offs` (optional): first token of every session in the packed call tensors, when the sessions are a SUBSET of the caller's
+// batch (a batch split by resume readiness, run_batch()); otherwise the sessions are packed back to back.
+static void build_schedule(ts_pool* pool, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
+                           const int32_t* q_offs = nullptr) {
   const ts_pool_config& c = pool->cfg;
   const int T = c.frame_tokens, H = c.n_heads, W = c.window_frames;
   std::vector<int64_t>& key = pool->scratch_key;
@@ -572,6 +582,7 @@ static void build_schedule(ts_pool* pool, int32_t n, const int32_t* sids, const 
     key.push_back(sids[b]);
     key.push_back(chunk_frames[b]);
     key.push_back((int64_t)pool->sess[sids[b]].ver);
+    key.push_back(q_offs ? q_offs[b] : -1);
   }
   if (key == pool->sched_key) return;
   const int grid_max = std::max(2, pool->sm_count & ~1);
@@ -589,7 +600,7 @@ static void build_schedule(ts_pool* pool, int32_t n, const int32_t* sids, const 
     const int C = cfr * T;
     const int a = W > 0 ? std::max(0, s.P + cfr - W) : 0;     // window start in frames (R6 i)
     SessDesc& d = sd[b];
-    d.q_off = q_off;
+    d.q_off = q_offs ? q_offs[b] : q_off;
     d.C = C;
     d.x_begin = s.o + a * T;
     d.x_end = s.o + s.P * T;
@@ -763,7 +774,7 @@ static void fill_block(ts_pool* pool, uint8_t* h, const BlockLayout& L, int n, c
 // Per-session 3D maps {D, H, C} of the call's packed Q / Kn / Vn: rows past a session's chunk read as zeros, never as a
 // neighbour's tokens.  `chunk_frames` fixes the geometry (q_off, C); nothing else of the schedule is needed.
 static bool encode_session_maps(ts_pool* pool, CUtensorMap* maps, int n, const int32_t* chunk_frames, const void* q,
-                                const void* k, const void* v) {
+                                const void* k, const void* v, const int32_t* q_offs = nullptr) {
   const ts_pool_config& c = pool->cfg;
   const int H = c.n_heads, D = c.head_dim;
   size_t q_off = 0;
@@ -773,7 +784,7 @@ static bool encode_session_maps(ts_pool* pool, CUtensorMap* maps, int n, const i
     const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)H * D * 2};
     const cuuint32_t box_q[3] = {64, 1, 128};
     const cuuint32_t box_kv[3] = {64, 1, (cuuint32_t)std::min(c.page_tokens, 64)};   // same box rows as the cache maps
-    const size_t byte_off = q_off * H * D * 2;
+    const size_t byte_off = (q_offs ? (size_t)q_offs[b] : q_off) * H * D * 2;
     if (!encode_map(&maps[b * 3 + 0], (uint8_t*)q + byte_off, 3, dims, strides, box_q)) return false;
     if (!encode_map(&maps[b * 3 + 1], (uint8_t*)k + byte_off, 3, dims, strides, box_kv)) return false;
     if (!encode_map(&maps[b * 3 + 2], (uint8_t*)v + byte_off, 3, dims, strides, box_kv)) return false;
@@ -886,9 +897,12 @@ static void ungrow(ts_pool* pool, int32_t n, const int32_t* sids, const FusedApp
 }
 
 // --------------------------------------------------------------------------------------------- attention
+// One launch for `n` sessions.  `cs` (optional): the append descriptors of a fused step, one per session; `q_offs` (optional):
+// see build_schedule.
 static int attention_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
-                          const void* q, const void* k, const void* v, void* out, float* lse, float scale,
-                          void* cuda_stream, const FusedAppend* fused, uint64_t* seq_out) {
+                          const int32_t* q_offs, const void* q, const void* k, const void* v, void* out, float* lse,
+                          float scale, void* cuda_stream, const CopySess* cs, uint64_t wait_side, uint64_t wait_compute,
+                          uint64_t* seq_out) {
   if (pool == nullptr) return TS_ERR_INVALID;
   int rc = check_batch(pool, layer, n, sids, chunk_frames);
   if (rc != TS_OK) return rc;
@@ -900,26 +914,29 @@ static int attention_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   TS_CUDA(cudaSetDevice(c.device));
 
-  build_schedule(pool, n, sids, chunk_frames);
+  build_schedule(pool, n, sids, chunk_frames, q_offs);
   const int grid = pool->sched_cta[0];
-  const BlockLayout L = block_layout(n, 1, pool->sched_pt.size(), pool->sched_items.size(), grid, fused != nullptr);
+  const BlockLayout L = block_layout(n, 1, pool->sched_pt.size(), pool->sched_items.size(), grid, cs != nullptr);
   Staging* st = nullptr;
   rc = acquire_staging(pool, L.bytes, &st);
   if (rc != TS_OK) return rc;
-  fill_block(pool, st->h, L, n, fused ? fused->cs.data() : nullptr);
-  if (!encode_session_maps(pool, reinterpret_cast<CUtensorMap*>(st->h + L.off_maps), n, chunk_frames, q, k, v)) return TS_ERR_CUDA;
+  fill_block(pool, st->h, L, n, cs);
+  if (!encode_session_maps(pool, reinterpret_cast<CUtensorMap*>(st->h + L.off_maps), n, chunk_frames, q, k, v, q_offs))
+    return TS_ERR_CUDA;
 
   // ---- ordering: wait (stream-side) for pending resumes of the batch's sessions
   for (int b = 0; b < n; ++b) TS_CUDA(pool->tl_side.wait(stream, pool->sess[sids[b]].side_seq));
-  if (fused) {   // ... and for copies out of / readers of the pages the append is about to write
-    TS_CUDA(pool->tl_side.wait(stream, fused->wait_side));
-    TS_CUDA(pool->tl_compute.wait(stream, fused->wait_compute));
+  if (cs != nullptr) {   // ... and for copies out of / readers of the pages the append is about to write
+    TS_CUDA(pool->tl_side.wait(stream, wait_side));
+    TS_CUDA(pool->tl_compute.wait(stream, wait_compute));
   }
 
   rc = upload_staging(pool, st, L.bytes, stream);
   if (rc != TS_OK) return rc;
-  const AttnParams p = make_params(pool, L, st->d, n, 0, layer, k, v, out, lse, scale, fused != nullptr,
-                                   fused ? fused->total_rows : 0);
+  int total_rows = 0;
+  if (cs != nullptr)
+    for (int b = 0; b < n; ++b) total_rows += cs[b].n_tok + cs[b].n_zero;
+  const AttnParams p = make_params(pool, L, st->d, n, 0, layer, k, v, out, lse, scale, cs != nullptr, total_rows);
   TS_CUDA(launch_attention(p, c.head_dim, grid, stream));
   ++pool->launches;
   TS_CUDA(cudaEventRecord(st->ev, stream));
@@ -930,9 +947,77 @@ static int attention_impl(ts_pool* pool, int32_t layer, int32_t n, const int32_t
   return TS_OK;
 }
 
+static void append_commit(ts_pool* pool, int32_t n, const int32_t* sids, const int32_t* chunk_frames, uint32_t flags,
+                          uint64_t seq);
+
+// PAPER.md:76 (iii) "restored ... before chunk generation resumes", without making the rest of the batch wait: when some
+// sessions of the batch still have a resume in flight on the side stream (and others do not), the batch runs as TWO launches -
+// the sessions that are ready first, the resuming ones behind their copy events - so that the ready sessions' attention hides
+// the copies instead of following them.  Results are those of one launch (sessions are independent); the packed
+// tensors are addressed through per-session offsets, so a group need not be contiguous in them.  `fa`: the fused append of
+// the whole batch (grown tables, descriptors in batch order) or null; with it, each group commits (`flags`) behind its own
+// launch.
+static int run_batch(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames, const void* q,
+                     const void* k, const void* v, void* out, float* lse, float scale, void* cuda_stream, const FusedAppend* fa,
+                     uint32_t flags, int* groups_done) {
+  *groups_done = 0;
+  std::vector<int32_t>& pend = pool->scratch_pending;   // decided ONCE: a resume may complete while the groups are being built
+  pend.assign(n, 0);
+  int n_pending = 0;
+  for (int b = 0; b < n; ++b) {
+    pend[b] = !pool->tl_side.is_done(pool->sess[sids[b]].side_seq);
+    n_pending += pend[b];
+  }
+  if (n_pending == 0 || n_pending == n) {
+    uint64_t seq = 0;
+    const int rc = attention_impl(pool, layer, n, sids, chunk_frames, nullptr, q, k, v, out, lse, scale, cuda_stream,
+                                  fa ? fa->cs.data() : nullptr, fa ? fa->wait_side : 0, fa ? fa->wait_compute : 0, &seq);
+    if (rc != TS_OK) return rc;
+    if (fa) append_commit(pool, n, sids, chunk_frames, flags, seq);
+    *groups_done = 1;
+    return TS_OK;
+  }
+  ++pool->split_batches;
+  std::vector<int32_t>& ss = pool->scratch_sub_sids;
+  std::vector<int32_t>& sc = pool->scratch_sub_cf;
+  std::vector<int32_t>& so = pool->scratch_sub_off;
+  std::vector<CopySess>& scs = pool->scratch_sub_cs;
+  for (int pass = 0; pass < 2; ++pass) {           // pass 0: the sessions that are ready; pass 1: the resuming ones
+    ss.clear();
+    sc.clear();
+    so.clear();
+    scs.clear();
+    int q_off = 0;
+    for (int b = 0; b < n; ++b) {
+      if (pend[b] == pass) {
+        ss.push_back(sids[b]);
+        sc.push_back(chunk_frames[b]);
+        so.push_back(q_off);
+        if (fa) scs.push_back(fa->cs[b]);
+      }
+      q_off += chunk_frames[b] * pool->cfg.frame_tokens;
+    }
+    uint64_t seq = 0;
+    const int rc = attention_impl(pool, layer, (int)ss.size(), ss.data(), sc.data(), so.data(), q, k, v, out, lse, scale,
+                                  cuda_stream, fa ? scs.data() : nullptr, fa ? fa->wait_side : 0, fa ? fa->wait_compute : 0, &seq);
+    if (rc != TS_OK) return rc;
+    if (fa) append_commit(pool, (int)ss.size(), ss.data(), sc.data(), flags, seq);
+    ++*groups_done;
+  }
+  return TS_OK;
+}
+
 int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
                        const void* q, const void* k, const void* v, void* out, float* lse, float scale, void* cuda_stream) {
-  return attention_impl(pool, layer, n, sids, chunk_frames, q, k, v, out, lse, scale, cuda_stream, nullptr, nullptr);
+  if (pool == nullptr) return TS_ERR_INVALID;
+  int rc = check_batch(pool, layer, n, sids, chunk_frames);
+  if (rc != TS_OK) return rc;
+  if (n == 0) return TS_OK;
+  if (q == nullptr || k == nullptr || v == nullptr || out == nullptr) return TS_ERR_INVALID;
+  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v) & 15) != 0 || ((uintptr_t)out & 31) != 0) return TS_ERR_INVALID;
+  if (!(scale > 0.0f) || !std::isfinite(scale)) return TS_ERR_INVALID;
+  int groups = 0;
+  return run_batch(pool, layer, n, sids, chunk_frames, q, k, v, out, lse, scale, cuda_stream, nullptr, 0, &groups);
 }
 
 // --------------------------------------------------------------------------------------------- append
@@ -1068,13 +1153,15 @@ int ts_chunk_step(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, 
   FusedAppend& fa = *pool->scratch_fused;   // (the vectors keep their capacity from call to call)
   fa.reset();
   grow_for_append(pool, n, sids, chunk_frames, &fa);
-  uint64_t seq = 0;
-  rc = attention_impl(pool, layer, n, sids, chunk_frames, q, k, v, out, lse, scale, cuda_stream, &fa, &seq);
+  int groups = 0;
+  rc = run_batch(pool, layer, n, sids, chunk_frames, q, k, v, out, lse, scale, cuda_stream, &fa, flags, &groups);
   if (rc != TS_OK) {
-    ungrow(pool, n, sids, fa);   // a CUDA failure on the way: the tables and the free list are as before the call
+    // a CUDA failure on the way.  Nothing enqueued yet: the tables and the free list are as before the call.  The first of
+    // two groups already running (a batch split by resume readiness): it stays committed, the tables of the second stay
+    // grown as after an uncommitted append.
+    if (groups == 0) ungrow(pool, n, sids, fa);
     return rc;
   }
-  append_commit(pool, n, sids, chunk_frames, flags, seq);
   return TS_OK;
 }
 

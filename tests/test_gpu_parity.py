@@ -832,3 +832,57 @@ def test_output_alignment_is_checked():
     torch.cuda.synchronize()
     assert torch.isfinite(good.float()).all()
     dp.g.close()
+
+
+@pytest.mark.parametrize("fused", [False, True])
+def test_batch_with_resumes_in_flight_runs_ready_sessions_first(fused):
+    """PAPER.md:76 (iii): sessions 1 and 3 of a five-session batch are resumed right before the call (their copies - ~10 MB
+    each - are still in flight when it is made): the call runs as two launches (ready sessions 0, 2, 4 first, then 1 and 3
+    behind their copy events; the groups are NOT contiguous in the packed tensors) and the result is that of one launch:
+    output against the oracle, appended bytes, page tables."""
+    import paper_2606_19271_b200 as tc
+    shape = shape_of(n_heads=4, head_dim=128, frame_tokens=200, window_frames=9, page_tokens=64, n_pages=5 * 40, max_sessions=8)
+    rng = np.random.default_rng(70 + int(fused))
+    dp = DualPool(shape, rng.permutation(shape.n_pages), host_pages=2 * 40)
+    T = shape.frame_tokens
+    sids = [dp.open() for _ in range(5)]
+    for i, sid in enumerate(sids):
+        n_frames = (6, 6, 2, 6, 0)[i]
+        if n_frames:
+            dp.feed_prior(sid, [draw(rng, n_frames * T, shape)], [draw(rng, n_frames * T, shape)])
+    cf = [2, 3, 1, 2, 3]
+    scale = scale_of(shape)
+    for step in range(3):
+        for sid in (sids[1], sids[3]):
+            dp.suspend(sid)
+        dp.g.ts_offload_sync()
+        torch.cuda.synchronize()
+        before = dp.g.ts_pool_split_batches()
+        # a long copy in front of the resumes on the side stream, so that they are certainly still pending at call time
+        blocker_h = torch.empty(256 << 20, dtype=torch.uint8).pin_memory()
+        blocker_d = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        q, k, v = (draw(rng, sum(cf) * T, shape) for _ in range(3))
+        # the oracle's side first (it takes seconds); then the GPU calls back to back, so that the resumes are still in flight
+        for sid in (sids[1], sids[3]):
+            dp.o.resume(sid)
+        o_ref, _ = oracle.chunk_attention(dp.o, 0, sids, cf, q, k, v, scale)
+        dp.o.append(0, sids, cf, k, v, commit=True)
+        dq, dk, dv = bits_to_dev(q), bits_to_dev(k), bits_to_dev(v)
+        out = torch.full_like(dq, float("nan"))
+        torch.cuda.synchronize()
+        with torch.cuda.stream(dp.g.side_stream):
+            blocker_d.copy_(blocker_h, non_blocking=True)
+        for sid in (sids[1], sids[3]):
+            dp.g.ts_session_resume(sid)
+        if fused:
+            dp.g.ts_chunk_step(0, sids, cf, dq, dk, dv, out, None, float(scale), tc.TS_COMMIT)
+        else:
+            dp.g.ts_chunk_attention(0, sids, cf, dq, dk, dv, out, None, float(scale))
+            dp.g.ts_kv_append(0, sids, cf, dk, dv, tc.TS_COMMIT)
+        torch.cuda.synchronize()
+        o_gpu = out.double().cpu().numpy()
+        assert np.isfinite(o_gpu).all()
+        assert np.abs(o_gpu - o_ref).max() <= 2e-2 and rel_l2(o_gpu, o_ref) <= 5e-3
+        assert dp.g.ts_pool_split_batches() == before + 1
+        dp.check_state(sids)
+    dp.g.close()
