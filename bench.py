@@ -4,7 +4,7 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras]
 
 One JSON line on stdout (rank 0).  A "step" is one pass of the hot path over one coalesced batch:
-    resume(idle session X) on the side stream                      (a6)
+    resume(idle session X) on the side stream                      (a6)   (suspends run on a second offload stream)
     open + close of a transient session                            (a7)
     every COMMIT_EVERY-th step: the transient session's first chunk as a real committed step - page growth, a
         schedule build for it AND (single-entry schedule cache) a rebuild for the main batch, commit (a1, a3, a4)
@@ -260,6 +260,7 @@ def join_side(pool):
     """Make the current stream wait for the pool's side stream (the step ends when both are done)."""
     import torch
     torch.cuda.current_stream().wait_stream(pool.side_stream)
+    torch.cuda.current_stream().wait_stream(pool.suspend_stream)
 
 
 # ------------------------------------------------------------------------------------------------ CPU baseline
@@ -748,25 +749,29 @@ def measure_overlap(wl, out, reps=12):
         b.record()
         torch.cuda.synchronize()
         alone.append(a.elapsed_time(b) / n_steps)
+    out_s = pool.suspend_stream
     for r in range(reps):
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        evs = [torch.cuda.Event(enable_timing=True) for _ in range(7)]
+        ev_in = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
+        ev_out = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
         a.record()
         side.wait_event(a)                     # the offload starts with the first step
-        evs[0].record(side)
-        for i in range(3):                     # 3 x (resume 201 MB H2D, suspend 201 MB D2H): ~25 ms of side-stream work
+        out_s.wait_event(a)
+        for i in range(3):                     # 3 x (resume 201 MB H2D, suspend 201 MB D2H): the two directions run at once
+            ev_in[2 * i].record(side)
             pool.ts_session_resume(y)
-            evs[2 * i + 1].record(side)
+            ev_in[2 * i + 1].record(side)
+            ev_out[2 * i].record(out_s)
             pool.ts_session_suspend(z)
-            evs[2 * i + 2].record(side)
+            ev_out[2 * i + 1].record(out_s)
             y, z = z, y
         for _ in range(n_steps):
             step()
         b.record()
         torch.cuda.synchronize()
         loaded.append(a.elapsed_time(b) / n_steps)
-        h2d_ms += [evs[2 * i].elapsed_time(evs[2 * i + 1]) for i in range(3)]
-        d2h_ms += [evs[2 * i + 1].elapsed_time(evs[2 * i + 2]) for i in range(3)]
+        h2d_ms += [ev_in[2 * i].elapsed_time(ev_in[2 * i + 1]) for i in range(3)]
+        d2h_ms += [ev_out[2 * i].elapsed_time(ev_out[2 * i + 1]) for i in range(3)]
     pool.close()
     alone_ms, loaded_ms = float(np.median(alone)), float(np.median(loaded))
     h2d, d2h = float(np.median(h2d_ms)), float(np.median(d2h_ms))
@@ -980,8 +985,8 @@ def run_config4(device, peak):
         torch.cuda.synchronize(device)
         t0 = time.perf_counter()
         moved = 0
-        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        s0.record(side)
+        s0, s1, s2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        s0.record()                                        # everything is idle here: the offload of the step starts now
         for u in ev["suspend"]:
             moved += pool.ts_session_info(sid_of[u])["n_pages"] * pool.page_bytes
             pool.ts_session_suspend(sid_of[u])
@@ -989,6 +994,7 @@ def run_config4(device, peak):
             pool.ts_session_resume(sid_of[u])
             moved += pool.ts_session_info(sid_of[u])["n_pages"] * pool.page_bytes
         s1.record(side)
+        s2.record(pool.suspend_stream)
         for u in ev["open"]:
             sid_of[u] = pool.ts_session_open()
             frames[u] = 0
@@ -1005,7 +1011,7 @@ def run_config4(device, peak):
         torch.cuda.synchronize(device)
         if moved:
             off_bytes += moved
-            off_ms += s0.elapsed_time(s1)
+            off_ms += max(s0.elapsed_time(s1), s0.elapsed_time(s2))   # the two directions run at the same time
         for u in ev["close"]:
             pool.ts_session_close(sid_of.pop(u))
             frames.pop(u)
@@ -1019,7 +1025,8 @@ def run_config4(device, peak):
             "attention_tflops_best_step": round(float((fl / lat_a).max() / 1e9), 1),
             "frac": round(float(fl.sum() / lat_a.sum() / 1e9) / peak, 4),
             "offload_gb": round(off_bytes / 1e9, 2), "offload_gbs": round(off_bytes / max(off_ms, 1e-9) / 1e6, 2),
-            "note": "latency includes the host calls and any resume the batch waits for; offload rate = bytes / side-stream time"}
+            "note": "latency includes the host calls and any resume the batch waits for; offload rate = bytes moved in both directions / time "
+                    "until both offload streams are done (suspends and resumes run on two streams, at the same time)"}
 
 
 def measure_offload(wl, permuted=False):
@@ -1045,21 +1052,23 @@ def measure_offload(wl, permuted=False):
         pool.ts_kv_append(0, [sid], [3], kk, kk, TS_COMMIT)
     n_pages = pool.ts_session_info(sid)["n_pages"]
     nbytes = n_pages * pool.page_bytes
-    side = pool.side_stream
+    side, out_s = pool.side_stream, pool.suspend_stream
     res = {}
     torch.cuda.synchronize()
     times = {"d2h": [], "h2d": []}
     for it in range(7):
-        a, b, c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
-        a.record(side)
-        pool.ts_session_suspend(sid)
-        b.record(side)
-        pool.ts_session_resume(sid)
+        a, b, b2, c = (torch.cuda.Event(enable_timing=True) for _ in range(4))
+        a.record(out_s)
+        pool.ts_session_suspend(sid)                      # device -> host on the suspend stream
+        b.record(out_s)
+        side.wait_event(b)
+        b2.record(side)
+        pool.ts_session_resume(sid)                       # host -> device on the side stream
         c.record(side)
         side.synchronize()
         if it:
             times["d2h"].append(a.elapsed_time(b))
-            times["h2d"].append(b.elapsed_time(c))
+            times["h2d"].append(b2.elapsed_time(c))
     # reference: one large pinned copy each way
     dbuf = torch.empty(nbytes, dtype=torch.uint8, device=dev)
     hbuf = torch.empty(nbytes, dtype=torch.uint8).pin_memory()

@@ -246,14 +246,17 @@ int ts_step_plan_destroy(ts_step_plan* plan);
 int64_t ts_step_plan_block_bytes(ts_step_plan* plan);
 
 /* PAPER.md:76 (i)-(ii): copy the session's pages (every layer, whole pages, logical order — R11) to the pinned
- * arena on the side stream, after the compute-stream work already enqueued on that session; mark SUSPENDED;
+ * arena on the pool's suspend stream, after the compute-stream work already enqueued on that session; mark SUSPENDED;
  * push its page ids to the back of the free list in logical order.  A freed page is not handed to a later
- * writer before the copy out of it has completed (event-ordered). */
+ * writer before the copy out of it has completed (event-ordered).  Suspends (device -> host) and resumes (host -> device)
+ * run on two streams of the pool, so that the two directions of the host link work at the same time; every dependency
+ * between them (a resume into pages a suspend is still reading, a suspend into arena slots a resume is still reading, the
+ * suspend and the resume of one session) is an event edge. */
 int ts_session_suspend(ts_pool* pool, int32_t sid);
 /* PAPER.md:76 (iii): pop the saved number of pages from the front of the free list, copy the host pages back
  * on the side stream, mark RESIDENT.  Later compute calls on the session wait (stream-side) for the copy. */
 int ts_session_resume(ts_pool* pool, int32_t sid);
-/* Host-blocks until all side-stream work enqueued so far has completed. */
+/* Host-blocks until all offload work (both streams) enqueued so far has completed. */
 int ts_offload_sync(ts_pool* pool);
 
 /*
@@ -288,8 +291,10 @@ int ts_gather_kv(ts_pool* pool, int32_t layer, int32_t sid, void* k_out, void* v
 /* Copies up to `cap` ids of the free list, front first. */
 int ts_pool_free_list(ts_pool* pool, int32_t* out, int32_t cap, int32_t* n_out);
 int ts_pool_stats(ts_pool* pool, ts_pool_stats_t* out);
-/* The side stream in use (cudaStream_t), for timing offload with events. */
+/* The offload streams in use (cudaStream_t), for timing offload with events: resumes and migration fetches run on the side
+ * stream (ts_pool_config.side_stream, or the pool's own), suspends on the suspend stream (always the pool's own). */
 void* ts_pool_side_stream(ts_pool* pool);
+void* ts_pool_suspend_stream(ts_pool* pool);
 /* Number of kernels the library has launched on this pool since creation, descriptor-upload kernels included
  * (bench.py's gpu_launches). */
 int64_t ts_pool_launch_count(ts_pool* pool);

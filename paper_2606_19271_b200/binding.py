@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = [
     "ts_pool_page_bytes", "ts_pool_slab_bytes", "ts_pool_create", "ts_pool_destroy", "ts_session_open",
     "ts_session_close", "ts_chunk_attention", "ts_kv_append", "ts_chunk_step", "ts_chunk_step_host", "ts_session_suspend",
     "ts_session_resume", "ts_session_migrate", "ts_offload_sync", "ts_session_info", "ts_session_page_table", "ts_gather_kv",
-    "ts_pool_free_list", "ts_pool_stats", "ts_pool_side_stream", "ts_pool_launch_count", "ts_pool_sched_builds", "ts_pool_split_batches",
+    "ts_pool_free_list", "ts_pool_stats", "ts_pool_side_stream", "ts_pool_suspend_stream", "ts_pool_launch_count", "ts_pool_sched_builds", "ts_pool_split_batches",
     "ts_pool_clock_probe", "ts_strerror",
     "ts_last_cuda_error", "ts_version",
     "ts_step_plan_create", "ts_step_plan_bind", "ts_step_plan_prepare", "ts_step_plan_run", "ts_step_plan_commit",
@@ -92,6 +92,8 @@ def _load():
     L.ts_pool_stats.argtypes = [P, C.POINTER(ts_pool_stats_t)]
     L.ts_pool_side_stream.restype = P
     L.ts_pool_side_stream.argtypes = [P]
+    L.ts_pool_suspend_stream.restype = P
+    L.ts_pool_suspend_stream.argtypes = [P]
     L.ts_pool_launch_count.restype = C.c_int64
     L.ts_pool_launch_count.argtypes = [P]
     L.ts_pool_sched_builds.restype = C.c_int64
@@ -340,7 +342,15 @@ class TurboChunkPool:
 
     @property
     def side_stream(self):
+        """The stream resumes (and migration fetches) run on."""
         return self._side
+
+    @property
+    def suspend_stream(self):
+        """The stream suspends run on (owned by the library), as a torch stream for event timing."""
+        if getattr(self, "_out", None) is None:
+            self._out = torch.cuda.ExternalStream(int(lib.ts_pool_suspend_stream(self._h)), device=self.device)
+        return self._out
 
 
 class StepPlan:

@@ -153,12 +153,16 @@ struct ts_pool {
   uint8_t* host = nullptr;
   bool own_host = false;
   int host_pages_cap = 0;
-  std::vector<int32_t> host_free;        // free arena slots (stack)
+  std::deque<int32_t> host_free;         // free arena slots, FIFO: a suspend takes the slots freed longest ago, not the ones a
+                                         // resume on the other offload stream may still be reading
   std::deque<int32_t> free_q;            // FIFO free list (R8)
   std::vector<uint64_t> page_compute_seq, page_side_seq;
   std::vector<Session> sess;
   cudaStream_t side = nullptr;
   bool own_side = false;
+  cudaStream_t side_out = nullptr;         // suspends (device -> host) run here, resumes (host -> device) on `side`: the host
+                                           // link is full duplex, one stream would put the two directions behind one another
+  std::vector<uint64_t> host_slot_seq;     // per arena slot: the resume (side timeline) that still reads it
   EventTimeline tl_compute, tl_side;
   std::vector<CUtensorMap> map_k, map_v;   // per layer
   int sm_count = 0;
@@ -357,6 +361,7 @@ int ts_pool_destroy(ts_pool* pool) {
   pool->tl_compute.sync_all();
   pool->tl_side.sync_all();
   if (pool->side) cudaStreamSynchronize(pool->side);
+  if (pool->side_out) cudaStreamSynchronize(pool->side_out);
   for (cudaStream_t st : {pool->up_s, pool->h2d_s, pool->d2h_s})
     if (st) cudaStreamSynchronize(st);
   for (Staging& s : pool->ring)
@@ -377,6 +382,7 @@ int ts_pool_destroy(ts_pool* pool) {
   pool->tl_compute.destroy();
   pool->tl_side.destroy();
   if (pool->own_side && pool->side) cudaStreamDestroy(pool->side);
+  if (pool->side_out) cudaStreamDestroy(pool->side_out);
   if (pool->own_slab && pool->slab) cudaFree(pool->slab);
   if (pool->own_host && pool->host) cudaFreeHost(pool->host);
   cudaGetLastError();
@@ -445,13 +451,15 @@ int ts_pool_create(const ts_pool_config* cfg, ts_pool** out) {
       pool->own_host = true;
     }
   }
-  for (int i = pool->host_pages_cap - 1; i >= 0; --i) pool->host_free.push_back(i);
+  for (int i = 0; i < pool->host_pages_cap; ++i) pool->host_free.push_back(i);
   if (cfg->side_stream != nullptr) {
     pool->side = (cudaStream_t)cfg->side_stream;
   } else {
     if (!cuda_ok(cudaStreamCreateWithFlags(&pool->side, cudaStreamNonBlocking), "cudaStreamCreate(side)")) return fail(TS_ERR_CUDA);
     pool->own_side = true;
   }
+  if (!cuda_ok(cudaStreamCreateWithFlags(&pool->side_out, cudaStreamNonBlocking), "cudaStreamCreate(side_out)")) return fail(TS_ERR_CUDA);
+  pool->host_slot_seq.assign(std::max(0, pool->host_pages_cap), 0);
   for (int i = 0; i < cfg->n_pages; ++i) pool->free_q.push_back(cfg->free_order ? cfg->free_order[i] : i);
   pool->page_compute_seq.assign(cfg->n_pages, 0);
   pool->page_side_seq.assign(cfg->n_pages, 0);
@@ -504,7 +512,10 @@ int ts_session_close(ts_pool* pool, int32_t sid) {
       pool->free_q.push_back(p);
     }
   } else {
-    for (auto it = s.host_slots.rbegin(); it != s.host_slots.rend(); ++it) pool->host_free.push_back(*it);
+    for (int32_t slot : s.host_slots) {
+      pool->host_slot_seq[slot] = s.side_seq;   // the copy out that fills the slot may still be running
+      pool->host_free.push_back(slot);
+    }
   }
   s = Session();
   return TS_OK;
@@ -556,6 +567,7 @@ int ts_pool_stats(ts_pool* pool, ts_pool_stats_t* out) {
 }
 
 void* ts_pool_side_stream(ts_pool* pool) { return pool ? (void*)pool->side : nullptr; }
+void* ts_pool_suspend_stream(ts_pool* pool) { return pool ? (void*)pool->side_out : nullptr; }
 int64_t ts_pool_sched_builds(ts_pool* pool) { return pool ? pool->sched_builds : 0; }
 int64_t ts_pool_split_batches(ts_pool* pool) { return pool ? pool->split_batches : 0; }
 int ts_pool_clock_probe(ts_pool* pool, void* device_u64x2) {
@@ -1424,7 +1436,7 @@ static int copy_session_pages(ts_pool* pool, const Session& s, bool to_host) {
     uint8_t* dev_ptr = pool->slab + (int64_t)s.pt[i] * pool->page_bytes;
     uint8_t* host_ptr = pool->host + (int64_t)s.host_slots[i] * pool->page_bytes;
     TS_CUDA(cudaMemcpyAsync(to_host ? host_ptr : dev_ptr, to_host ? dev_ptr : host_ptr, (size_t)(e - i) * pool->page_bytes, kind,
-                            pool->side));
+                            to_host ? pool->side_out : pool->side));
     i = e;
   }
   return TS_OK;
@@ -1439,18 +1451,24 @@ int ts_session_suspend(ts_pool* pool, int32_t sid) {
   if (s.in_plan) return TS_ERR_STATE;   // chunk-boundary rule (R12): not inside a prepared step
   if (s.pt.size() > pool->host_free.size()) return TS_ERR_NO_HOST;
   TS_CUDA(cudaSetDevice(c.device));
-  // chunk-boundary rule (R12): the copy out starts after the compute work already enqueued on the session
-  TS_CUDA(pool->tl_compute.wait(pool->side, s.compute_seq));
+  // chunk-boundary rule (R12): the copy out starts after the compute work already enqueued on the session - and after a
+  // resume of it that may still be copying in (resumes run on the other offload stream)
+  TS_CUDA(pool->tl_compute.wait(pool->side_out, s.compute_seq));
+  TS_CUDA(pool->tl_side.wait(pool->side_out, s.side_seq));
   s.host_slots.clear();
+  uint64_t wait_slots = 0;
   for (size_t i = 0; i < s.pt.size(); ++i) {
-    s.host_slots.push_back(pool->host_free.back());
-    pool->host_free.pop_back();
+    const int32_t slot = pool->host_free.front();
+    pool->host_free.pop_front();
+    wait_slots = std::max(wait_slots, pool->host_slot_seq[slot]);   // a resume may still be reading the slot
+    s.host_slots.push_back(slot);
   }
+  TS_CUDA(pool->tl_side.wait(pool->side_out, wait_slots));
   {
     const int rc = copy_session_pages(pool, s, true);
     if (rc != TS_OK) return rc;
   }
-  const uint64_t seq = pool->tl_side.record(pool->side);
+  const uint64_t seq = pool->tl_side.record(pool->side_out);
   for (int32_t pg : s.pt) {
     pool->page_side_seq[pg] = seq;
     pool->page_compute_seq[pg] = s.compute_seq;
@@ -1469,20 +1487,25 @@ int ts_session_resume(ts_pool* pool, int32_t sid) {
   Session& s = pool->sess[sid];
   if (s.host_slots.size() > pool->free_q.size()) return TS_ERR_NO_PAGES;
   TS_CUDA(cudaSetDevice(c.device));
-  uint64_t wait_compute = 0;
+  uint64_t wait_compute = 0, wait_side = s.side_seq;                     // its own copy out comes first
   for (size_t i = 0; i < s.host_slots.size(); ++i) {
     const int32_t pg = pool->free_q.front();
     pool->free_q.pop_front();
     wait_compute = std::max(wait_compute, pool->page_compute_seq[pg]);   // readers of the page's previous owner
+    wait_side = std::max(wait_side, pool->page_side_seq[pg]);            // ... and a copy out of it still in flight
     s.pt.push_back(pg);
   }
   TS_CUDA(pool->tl_compute.wait(pool->side, wait_compute));
+  TS_CUDA(pool->tl_side.wait(pool->side, wait_side));
   {
     const int rc = copy_session_pages(pool, s, false);
     if (rc != TS_OK) return rc;
   }
   s.side_seq = pool->tl_side.record(pool->side);
-  for (auto it = s.host_slots.rbegin(); it != s.host_slots.rend(); ++it) pool->host_free.push_back(*it);
+  for (int32_t slot : s.host_slots) {
+    pool->host_slot_seq[slot] = s.side_seq;                              // the slot may be overwritten after this copy
+    pool->host_free.push_back(slot);
+  }
   s.host_slots.clear();
   s.ver = ++pool->ver_seq;
   s.state = TS_SESSION_RESIDENT;
@@ -1528,12 +1551,13 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
   t = Session();
   t.P = s.P;
   t.o = s.o;
-  uint64_t wait_compute = 0;
+  uint64_t wait_compute = 0, wait_dst_side = 0;
   for (size_t i = 0; i < n; ++i) {
     const int32_t pg = dst->free_q.front();
     dst->free_q.pop_front();
     wait_compute = std::max(wait_compute, dst->page_compute_seq[pg]);   // readers of the page's previous owner
-    t.pt.push_back(pg);                                                 // (copies out of it are on this side stream)
+    wait_dst_side = std::max(wait_dst_side, dst->page_side_seq[pg]);    // ... and a copy out of it still in flight
+    t.pt.push_back(pg);
   }
   auto undo = [&]() {
     for (auto it = t.pt.rbegin(); it != t.pt.rend(); ++it) dst->free_q.push_front(*it);
@@ -1556,6 +1580,7 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
     TS_CUDA_UNDO(src->tl_compute.wait(dst->side, s.compute_seq));
     TS_CUDA_UNDO(src->tl_side.wait(dst->side, s.side_seq));
     TS_CUDA_UNDO(dst->tl_compute.wait(dst->side, wait_compute));
+    TS_CUDA_UNDO(dst->tl_side.wait(dst->side, wait_dst_side));
     TS_CUDA_UNDO(launch_upload(st->h_dev, st->d, align_up(n * 8, 16), dst->side));   // not a DMA copy: see upload_staging
     ++dst->launches;
     PullParams p;
@@ -1593,6 +1618,7 @@ int ts_offload_sync(ts_pool* pool) {
   if (pool == nullptr) return TS_ERR_INVALID;
   TS_CUDA(cudaSetDevice(pool->cfg.device));
   TS_CUDA(cudaStreamSynchronize(pool->side));
+  TS_CUDA(cudaStreamSynchronize(pool->side_out));
   return TS_OK;
 }
 
