@@ -146,6 +146,32 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
                        void* out, float* lse, float scale, void* cuda_stream);
 
 /*
+ * ts_chunk_attention (PAPER.md:66 (i)-(iii), same arguments, same result) for callers that cannot allocate: code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The call makes no cudaMalloc, cudaFree,
+ * cudaHostAlloc or event creation: the launch's schedule block (per-session tensor maps, session descriptors, packed page
+ * tables, work items and the kernel's work-item cursor and feed rings) lives in ONE array of ts_static_scratch_bytes()
+ * (256 KiB) bytes built into the library's device image - every GPU that loads the library holds it until the process
+ * exits - and reaches it by one cudaMemcpyAsync from ordinary host memory on `cuda_stream`, followed by the one launch.
+ * Limits and rules that ts_chunk_attention does not have:
+ *   - TS_ERR_CAPACITY (ts_last_cuda_error() names both sizes) when the batch's block does not fit the array; nothing was
+ *     enqueued.  53 KB for configs[2] (8 sessions x 12 heads), ~160 KB for 32 such sessions.
+ *   - All calls on a device SHARE the array, which keeps the last call's contents: every call rewrites the whole block, the
+ *     cursor and the rings as zeros, so nothing is inherited - but two calls whose GPU work can overlap (different streams,
+ *     or different pools on one device, without an event between them) race on it.  One stream, or the caller's own
+ *     event edges, is the rule; host threads are serialised by the library.
+ *   - The call is not entered into the pool's event timelines: a session with a resume still copying in, or inside a step
+ *     plan, is TS_ERR_STATE (no stream-side wait), and the caller must let the call's work complete (or order it by its
+ *     own events) before it suspends, closes or migrates a session of the batch.
+ *   - The host may wait for work already in `cuda_stream` (the block is copied from pageable memory).
+ * Other errors as ts_chunk_attention.  Does not change pool state (R5).  n == 0 is a no-op.
+ */
+int ts_chunk_attention_static(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*host*/,
+                              const int32_t* chunk_frames /*host*/, const void* q, const void* k, const void* v,
+                              void* out, float* lse, float scale, void* cuda_stream);
+/* Size in bytes of the static device scratch array behind ts_chunk_attention_static. */
+int64_t ts_static_scratch_bytes(void);
+
+/*
  * PAPER.md:66 (iii) "writes the generated chunks and updated states back to their corresponding sessions".
  * Sessions in sids order: grow PT by ceil((o+L+C)/B) - |PT| pages popped from the front of the free list
  * (idempotent across the layers of one step), scatter the chunk's K/V to logical positions [L, L+C) of

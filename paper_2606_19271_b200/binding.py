@@ -26,6 +26,7 @@ EXPORTED_SYMBOLS = [
     "ts_last_cuda_error", "ts_version",
     "ts_step_plan_create", "ts_step_plan_bind", "ts_step_plan_prepare", "ts_step_plan_run", "ts_step_plan_commit",
     "ts_step_plan_destroy", "ts_step_plan_block_bytes",
+    "ts_chunk_attention_static", "ts_static_scratch_bytes",
     "ts_sched_create", "ts_sched_destroy", "ts_sched_event", "ts_sched_moves", "ts_sched_alive",
 ]
 
@@ -78,6 +79,9 @@ def _load():
     L.ts_session_open.argtypes = [P, I32P]
     L.ts_session_close.argtypes = [P, C.c_int32]
     L.ts_chunk_attention.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, P, P, P, C.c_float, P]
+    L.ts_chunk_attention_static.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, P, P, P, C.c_float, P]
+    L.ts_static_scratch_bytes.restype = C.c_int64
+    L.ts_static_scratch_bytes.argtypes = []
     L.ts_kv_append.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, C.c_uint32, P]
     L.ts_chunk_step.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, P, P, P, C.c_float, C.c_uint32, P]
     L.ts_chunk_step_host.argtypes = [P, C.c_int32, C.c_int32, I32P, I32P, P, P, P, P, C.c_float, C.c_uint32, P]
@@ -257,6 +261,15 @@ class TurboChunkPool:
         _check(lib.ts_chunk_attention(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(q), _ptr(k),
                                       _ptr(v), _ptr(out), _ptr(lse), C.c_float(float(scale)), _stream(stream, self.device)),
                "ts_chunk_attention")
+
+    def ts_chunk_attention_static(self, layer, sids, chunk_frames, q, k, v, out, lse=None, scale=1.0, stream=None):
+        """ts_chunk_attention without any allocation: the schedule block lives in the library's static device array."""
+        rc = lib.ts_chunk_attention_static(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(q), _ptr(k),
+                                           _ptr(v), _ptr(out), _ptr(lse), C.c_float(float(scale)),
+                                           _stream(stream, self.device))
+        if rc == TS_ERR_CAPACITY:   # the library says which size exceeded which limit
+            raise TurboChunkError(rc, lib.ts_last_cuda_error().decode())
+        _check(rc, "ts_chunk_attention_static")
 
     def ts_kv_append(self, layer, sids, chunk_frames, k, v, flags=TS_COMMIT, stream=None):
         _check(lib.ts_kv_append(self._h, layer, len(sids), _i32(sids), _i32(chunk_frames), _ptr(k), _ptr(v),

@@ -10,7 +10,9 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <queue>
 #include <string>
 
@@ -1692,6 +1694,97 @@ int ts_chunk_step_host(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
   TS_CUDA(cudaEventRecord(pool->ev_out, pool->d2h_s));
   TS_CUDA(cudaStreamWaitEvent(stream, pool->ev_out, 0));   // stream order: out_host is complete when the call is
   TS_CUDA(cudaEventRecord(pool->ev_free[slot], stream));   // ... and the staging set is free again
+  return TS_OK;
+}
+
+}  // extern "C"
+
+// --------------------------------------------------------------------------------------------- allocation-free attention
+// ts_chunk_attention_static: ts_chunk_attention for callers that cannot allocate (CUDA graph capture around the call,
+// tight serving loops, harnesses that forbid cudaMalloc).  The launch's schedule block - per-session tensor maps, session
+// descriptors, packed page tables, the work-item list and the kernel's work-item cursor and per-cluster feed rings (the only
+// part the kernel WRITES: scratch that has to be zero at launch) - does not go through the pool's staging ring (whose
+// buffers are cudaMalloc'ed and grow on demand) but into ONE file-scope device array of a fixed size.  Every GPU that loads
+// the library holds these kStaticScratchBytes until the process exits.
+//
+// In host code `g_static_scratch` is a host-side stand-in for the symbol, not a device address: the address the kernel
+// gets is looked up per device with cudaGetSymbolAddress, once, with that device current (static_scratch_ptr()).
+constexpr size_t kStaticScratchBytes = 256 * 1024;   // 32 Wan-1.3B-shaped sessions need ~160 KB, configs[2] 53 KB
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+namespace {
+
+std::mutex g_static_mu;                               // the host image below and the per-device addresses
+unsigned char* g_static_dev[64] = {};                 // device address of g_static_scratch on device i (null: not looked up yet)
+alignas(256) unsigned char g_static_host[kStaticScratchBytes];   // the block is assembled here (ordinary host memory)
+
+// Set-up, once per device, with that device current.  Allocates nothing: the array exists from the moment the library's
+// module is loaded on the device.
+int static_scratch_ptr(int device, unsigned char** out) {
+  if (device < 0 || device >= 64) return TS_ERR_INVALID;
+  if (g_static_dev[device] == nullptr) {
+    void* ptr = nullptr;
+    if (!tc::cuda_ok(cudaSetDevice(device), "cudaSetDevice(static scratch)")) return TS_ERR_CUDA;
+    if (!tc::cuda_ok(cudaGetSymbolAddress(&ptr, g_static_scratch), "cudaGetSymbolAddress(g_static_scratch)")) return TS_ERR_CUDA;
+    if (ptr == nullptr || ((uintptr_t)ptr & 255) != 0) {
+      tc::g_last_cuda_error = "cudaGetSymbolAddress(g_static_scratch): null or misaligned device address";
+      return TS_ERR_CUDA;
+    }
+    g_static_dev[device] = (unsigned char*)ptr;
+  }
+  *out = g_static_dev[device];
+  return TS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int64_t ts_static_scratch_bytes(void) { return (int64_t)kStaticScratchBytes; }
+
+int ts_chunk_attention_static(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids, const int32_t* chunk_frames,
+                              const void* q, const void* k, const void* v, void* out, float* lse, float scale,
+                              void* cuda_stream) {
+  if (pool == nullptr) return TS_ERR_INVALID;
+  int rc = check_batch(pool, layer, n, sids, chunk_frames);
+  if (rc != TS_OK) return rc;
+  if (n == 0) return TS_OK;
+  if (q == nullptr || k == nullptr || v == nullptr || out == nullptr) return TS_ERR_INVALID;
+  if ((((uintptr_t)q | (uintptr_t)k | (uintptr_t)v) & 15) != 0 || ((uintptr_t)out & 31) != 0) return TS_ERR_INVALID;
+  if (!(scale > 0.0f) || !std::isfinite(scale)) return TS_ERR_INVALID;
+  const ts_pool_config& c = pool->cfg;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  // This call stays outside the pool's event timelines (recording into them creates events on demand, and an event recorded
+  // under stream capture cannot be waited for outside the graph): a session with a resume still copying in is refused.
+  for (int b = 0; b < n; ++b) {
+    const Session& s = pool->sess[sids[b]];
+    if (s.in_plan || !pool->tl_side.is_done(s.side_seq)) return TS_ERR_STATE;
+  }
+  TS_CUDA(cudaSetDevice(c.device));
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  unsigned char* d = nullptr;
+  rc = static_scratch_ptr(c.device, &d);
+  if (rc != TS_OK) return rc;
+
+  build_schedule(pool, n, sids, chunk_frames);
+  const int grid = pool->sched_cta[0];
+  const BlockLayout L = block_layout(n, 1, pool->sched_pt.size(), pool->sched_items.size(), grid, false);
+  if (L.bytes > kStaticScratchBytes) {
+    char msg[200];
+    snprintf(msg, sizeof msg, "ts_chunk_attention_static: the batch's schedule block needs %zu bytes, the static scratch array holds %zu",
+             L.bytes, kStaticScratchBytes);
+    tc::g_last_cuda_error = msg;
+    return TS_ERR_CAPACITY;
+  }
+  // The whole block is rewritten by every call, the cursor and the feed rings as zeros (fill_block): nothing of the previous
+  // call's contents is relied on.  The source is ordinary host memory: the copy has left it when cudaMemcpyAsync returns.
+  fill_block(pool, g_static_host, L, n, nullptr);
+  if (!encode_session_maps(pool, reinterpret_cast<CUtensorMap*>(g_static_host + L.off_maps), n, chunk_frames, q, k, v))
+    return TS_ERR_CUDA;
+  TS_CUDA(cudaMemcpyAsync(d, g_static_host, align_up(L.bytes, 16), cudaMemcpyHostToDevice, stream));
+  const AttnParams p = make_params(pool, L, d, n, 0, layer, k, v, out, lse, scale, false, 0);
+  TS_CUDA(launch_attention(p, c.head_dim, grid, stream));
+  ++pool->launches;
   return TS_OK;
 }
 
