@@ -146,8 +146,9 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
                        void* out, float* lse, float scale, void* cuda_stream);
 
 /*
- * ts_chunk_attention (PAPER.md:66 (i)-(iii), same arguments, same result) for callers that cannot allocate: code under CUDA
- * graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The call makes no cudaMalloc, cudaFree,
+ * ts_chunk_attention (PAPER.md:66 (i)-(iii), same arguments, same result) for callers that cannot allocate: a process with
+ * a CUDA graph capture in progress (cudaMalloc is illegal then in the default capture mode), tight serving loops, harnesses
+ * that forbid cudaMalloc.  The call makes no cudaMalloc, cudaFree,
  * cudaHostAlloc or event creation: the launch's schedule block (per-session tensor maps, session descriptors, packed page
  * tables, work items and the kernel's work-item cursor and feed rings) lives in ONE array of ts_static_scratch_bytes()
  * (256 KiB) bytes built into the library's device image - every GPU that loads the library holds it until the process
@@ -163,6 +164,8 @@ int ts_chunk_attention(ts_pool* pool, int32_t layer, int32_t n, const int32_t* s
  *     plan, is TS_ERR_STATE (no stream-side wait), and the caller must let the call's work complete (or order it by its
  *     own events) before it suspends, closes or migrates a session of the batch.
  *   - The host may wait for work already in `cuda_stream` (the block is copied from pageable memory).
+ *   - Do not capture the call itself into a graph: the copy would become a node that re-reads, at every replay, a host image
+ *     the next call overwrites.  ts_step_plan_run is the capturable launch.
  * Other errors as ts_chunk_attention.  Does not change pool state (R5).  n == 0 is a no-op.
  */
 int ts_chunk_attention_static(ts_pool* pool, int32_t layer, int32_t n, const int32_t* sids /*host*/,
