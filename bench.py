@@ -478,6 +478,8 @@ def main():
     result["offload"]["scattered"] = {k: v for k, v in measure_offload(wl, permuted=True).items()
                                       if k in ("d2h", "h2d", "placement")}
     result["migrate"] = measure_migration(wl, peaks["hbm_gbs"])
+    if extras:
+        result["migrate_ipc"] = measure_migration_ipc(wl, peaks["hbm_gbs"])
     if world > 1 and torch.cuda.device_count() >= 2:
         result["migrate_p2p"] = measure_migration_p2p(wl)
     if extras:
@@ -1139,6 +1141,66 @@ def measure_migration(wl, hbm_peak):
             "algorithmic_bytes_per_launch": int(2 * nbytes), "ms_per_move": round(best, 4), "achieved": round(gbs, 1),
             "peak": hbm_peak, "unit": "GB/s", "frac": round(gbs / hbm_peak, 4),
             "note": "both pools on this GPU (read + write in HBM); across GPUs the fetch reads over NVLink"}
+
+
+def measure_migration_ipc(wl, hbm_peak):
+    """The same full-window session moved between two WORKER PROCESSES on this GPU (paper_2606_19271_b200.worker: one pool
+    each, the source slab mapped through CUDA IPC, "state frozen" / "installed" as interprocess events; PAPER.md:263-265,
+    :271).  Reported: the device time of the fetches (4 sessions fetched back to back, events on the target's side stream)
+    and the wall-clock time of one whole move as the control plane sees it (freeze -> ticket -> import -> release: three
+    pipe round trips between three Python processes; no host synchronisation with the GPU in either worker)."""
+    import time
+    from paper_2606_19271_b200 import TS_COMMIT, worker
+    sh = wl["w"].shape
+    geo = dict(n_layers=1, n_heads=sh.n_heads, head_dim=sh.head_dim, page_tokens=sh.page_tokens, n_pages=4 * 132,
+               frame_tokens=sh.frame_tokens, window_frames=sh.window_frames, max_sessions=4)
+    ws = [worker.spawn(device=wl["q"].device.index or 0) for _ in range(2)]
+    try:
+        for w in ws:
+            w.post("create", **geo)
+        for w in ws:
+            w.result()
+        blobs = [w.call("pool", "ts_pool_export") for w in ws]
+        peers = [ws[0].call("pool", "ts_peer_open", blobs[1]), ws[1].call("pool", "ts_peer_open", blobs[0])]   # peer of the OTHER side
+        sids = [ws[0].call("pool", "ts_session_open") for _ in range(4)]
+        for i in range(7):
+            ws[0].call("append_random", 0, sids, [3] * 4, 200 + i, TS_COMMIT)
+        ws[0].call("sync")
+        n_pages = ws[0].call("pool", "ts_session_info", sids[0])["n_pages"]
+        nbytes = n_pages * ws[0].call("pool", "ts_pool_stats")["page_bytes"]
+        best_ms, walls = 1e9, []
+        where = 0
+        for rep in range(8):
+            src, dst = ws[where], ws[where ^ 1]
+            if rep < 4:      # device time: the four fetches enqueued back to back, events on the target's side stream
+                tickets = [src.call("pool", "ts_session_freeze", s) for s in sids]
+                new, ms = dst.call("timed_imports", peers[where ^ 1], tickets)
+                for s in sids:
+                    src.call("pool", "ts_session_release", s, peers[where])
+                if rep > 0:
+                    best_ms = min(best_ms, ms / len(sids))
+            else:            # control-plane time: whole moves one after the other, nothing waits for the GPU
+                new = []
+                for s in sids:
+                    t0 = time.perf_counter()
+                    ticket = src.call("pool", "ts_session_freeze", s)
+                    new.append(dst.call("pool", "ts_session_import", peers[where ^ 1], ticket))
+                    src.call("pool", "ts_session_release", s, peers[where])
+                    walls.append(time.perf_counter() - t0)
+            sids, where = new, where ^ 1
+        for w in ws:
+            w.call("sync")
+    finally:
+        for w in ws:
+            w.close()
+    gbs = 2 * nbytes / (best_ms * 1e-3) / 1e9
+    return {"bound": "hbm", "kernel": "page_pull_kernel (source slab through CUDA IPC)", "bytes_moved": int(nbytes),
+            "pages": int(n_pages), "algorithmic_bytes_per_launch": int(2 * nbytes), "ms_per_move_device": round(best_ms, 4),
+            "achieved": round(gbs, 1), "peak": hbm_peak, "unit": "GB/s", "frac": round(gbs / hbm_peak, 4),
+            "ms_per_move_control_plane": {"median": round(1e3 * sorted(walls)[len(walls) // 2], 3), "max": round(1e3 * max(walls), 3)},
+            "note": "two worker processes on this one GPU; device time = fetches of 4 sessions back to back on the target's "
+                    "side stream; control-plane time = wall clock of freeze + import + release per session through the "
+                    "parent's pipes (Python), no host-GPU synchronisation in the workers"}
 
 
 def measure_migration_p2p(wl, peer_peak_gbs=770.0):

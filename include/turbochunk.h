@@ -311,6 +311,62 @@ int ts_offload_sync(ts_pool* pool);
  */
 int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out);
 
+/*
+ * The same move between two WORKER PROCESSES (PAPER.md:66, :271: one worker per GPU; :263 "registers the corresponding
+ * state buffers ... the target worker can then fetch the registered state buffers from the source worker through ...
+ * one-sided GPU memory access"; :265 (i) freeze, (ii) fetch + verify, (iii) ownership flips after the transfer).  The two
+ * pools live in two processes, on one GPU or on two GPUs of a node with peer access; CUDA IPC makes the source slab an
+ * ordinary device pointer for the target's fetch kernel, and every GPU-side dependency is an interprocess event edge - no
+ * host wait in either process.  What travels between the processes (the "control plane": a pipe, a socket - not this
+ * library's business) is plain bytes, and must be delivered in order:
+ *   registration, once per pair of workers:  ts_pool_export on each side -> the blob -> ts_peer_open on the other side
+ *   per move:  source ts_session_freeze -> ticket + page ids -> target ts_session_import -> "enqueued" (any message)
+ *              -> source ts_session_release.
+ * Result and id / page-order rules exactly as ts_session_migrate (R22): the target installs the session under its lowest
+ * free id with |PT| pages popped from the front of its free list; the source's page ids go to the back of its free list
+ * in logical order when it releases.
+ *
+ * ts_pool_export  : fills `out` (opaque bytes: IPC handles of the slab's allocation and of two interprocess events,
+ *                   geometry).  The slab must come from cudaMalloc (the pool's own, or a caller slab inside a cudaMalloc
+ *                   allocation - not from a virtual-memory allocator).  Idempotent.  TS_ERR_CUDA if IPC is unavailable.
+ * ts_peer_open    : maps the remote slab into `local`'s process; TS_ERR_INVALID if the blob is malformed or the geometry
+ *                   (NL, H, D, B, T, W) differs from `local`'s.  A blob cannot be opened in the process that exported it.
+ * ts_peer_close   : waits for `local`'s side stream, then unmaps.
+ * ts_session_freeze : (i).  sid RESIDENT and not held by a step plan (else TS_ERR_STATE).  Records "state frozen" on the
+ *                   source's side stream behind the compute work already enqueued on the session; from here until
+ *                   release / unfreeze every other call on the session is TS_ERR_STATE.  Writes the ticket and the
+ *                   session's page ids in logical order (`cap` >= n_pages, else TS_ERR_INVALID and nothing changes).
+ * ts_session_unfreeze : the move is called off (the target had no room): the session is RESIDENT again.
+ * ts_session_import : (ii).  `source` = ts_peer_open of the source's blob on `dst`.  Verifies the ticket against the
+ *                   geometry (o < B, P <= W, n_pages * B >= o + P * T, every page id inside the source slab:
+ *                   TS_ERR_INVALID), then as the target half of ts_session_migrate: TS_ERR_CAPACITY, TS_ERR_NO_PAGES,
+ *                   TS_ERR_CUDA leave `dst` unchanged.  The fetch (one kernel on dst's side stream) waits for the source's
+ *                   "state frozen"; compute calls on the new session wait for the fetch; "installed" is recorded behind it.
+ * ts_session_release : (iii).  `target` = ts_peer_open of the target's blob on `src` (NULL: the caller itself guarantees
+ *                   that the fetch has completed).  The source's side stream waits for the target's "installed" before
+ *                   the freed pages can be handed to a writer; the session id is free again.  Call it only after the
+ *                   target has returned from ts_session_import.
+ */
+#define TS_POOL_EXPORT_BYTES 320
+typedef struct ts_pool_export_t {
+  unsigned char bytes[TS_POOL_EXPORT_BYTES];
+} ts_pool_export_t;
+typedef struct ts_migration_ticket_t {
+  int32_t sid;       /* id at the source (for ts_session_release / ts_session_unfreeze) */
+  int32_t frames;    /* P */
+  int32_t head_off;  /* o */
+  int32_t n_pages;   /* |PT| */
+} ts_migration_ticket_t;
+typedef struct ts_peer ts_peer;
+int ts_pool_export(ts_pool* pool, ts_pool_export_t* out);
+int ts_peer_open(ts_pool* local, const ts_pool_export_t* remote, ts_peer** out);
+int ts_peer_close(ts_peer* peer);
+int ts_session_freeze(ts_pool* src, int32_t sid, ts_migration_ticket_t* ticket, int32_t* pages_out /*host*/, int32_t cap);
+int ts_session_unfreeze(ts_pool* src, int32_t sid);
+int ts_session_import(ts_pool* dst, ts_peer* source, const ts_migration_ticket_t* ticket, const int32_t* pages /*host*/,
+                      int32_t* sid_out);
+int ts_session_release(ts_pool* src, int32_t sid, ts_peer* target /*nullable*/);
+
 /* Introspection (parity is taken on these, never on raw slabs: the physical layout is private). */
 int ts_session_info(ts_pool* pool, int32_t sid, ts_session_info_t* out);
 /* Copies up to `cap` page ids (logical order) to `out` (host); *n_out = |PT|. */

@@ -27,6 +27,8 @@ EXPORTED_SYMBOLS = [
     "ts_step_plan_create", "ts_step_plan_bind", "ts_step_plan_prepare", "ts_step_plan_run", "ts_step_plan_commit",
     "ts_step_plan_destroy", "ts_step_plan_block_bytes",
     "ts_chunk_attention_static", "ts_static_scratch_bytes",
+    "ts_pool_export", "ts_peer_open", "ts_peer_close", "ts_session_freeze", "ts_session_unfreeze", "ts_session_import",
+    "ts_session_release",
     "ts_sched_create", "ts_sched_destroy", "ts_sched_event", "ts_sched_moves", "ts_sched_alive",
 ]
 
@@ -42,6 +44,14 @@ class ts_pool_config(C.Structure):
 class ts_session_info_t(C.Structure):
     _fields_ = [("state", C.c_int32), ("frames", C.c_int32), ("len_tokens", C.c_int64), ("head_off", C.c_int32),
                 ("n_pages", C.c_int32)]
+
+
+class ts_pool_export_t(C.Structure):
+    _fields_ = [("bytes", C.c_ubyte * 320)]
+
+
+class ts_migration_ticket_t(C.Structure):
+    _fields_ = [("sid", C.c_int32), ("frames", C.c_int32), ("head_off", C.c_int32), ("n_pages", C.c_int32)]
 
 
 class ts_pool_stats_t(C.Structure):
@@ -89,6 +99,13 @@ def _load():
     L.ts_session_resume.argtypes = [P, C.c_int32]
     L.ts_session_migrate.argtypes = [P, C.c_int32, P, I32P]
     L.ts_offload_sync.argtypes = [P]
+    L.ts_pool_export.argtypes = [P, C.POINTER(ts_pool_export_t)]
+    L.ts_peer_open.argtypes = [P, C.POINTER(ts_pool_export_t), C.POINTER(P)]
+    L.ts_peer_close.argtypes = [P]
+    L.ts_session_freeze.argtypes = [P, C.c_int32, C.POINTER(ts_migration_ticket_t), I32P, C.c_int32]
+    L.ts_session_unfreeze.argtypes = [P, C.c_int32]
+    L.ts_session_import.argtypes = [P, P, C.POINTER(ts_migration_ticket_t), I32P, I32P]
+    L.ts_session_release.argtypes = [P, C.c_int32, P]
     L.ts_session_info.argtypes = [P, C.c_int32, C.POINTER(ts_session_info_t)]
     L.ts_session_page_table.argtypes = [P, C.c_int32, I32P, C.c_int32, I32P]
     L.ts_gather_kv.argtypes = [P, C.c_int32, C.c_int32, P, P, P]
@@ -211,6 +228,7 @@ class TurboChunkPool:
         handle = C.c_void_p()
         _check(lib.ts_pool_create(C.byref(cfg), C.byref(handle)), "ts_pool_create")
         self._h = handle
+        self._peers = []     # ts_peer handles opened on this pool (closed with it)
 
     def check_guards(self):
         """True if the guard bands around the KV slab and the pinned arena still hold their fill pattern."""
@@ -239,6 +257,9 @@ class TurboChunkPool:
     # ---- lifecycle
     def close(self):
         if getattr(self, "_h", None):
+            for peer in list(getattr(self, "_peers", [])):
+                lib.ts_peer_close(C.c_void_p(peer))
+            self._peers = []
             lib.ts_pool_destroy(self._h)
             self._h = None
 
@@ -304,6 +325,51 @@ class TurboChunkPool:
 
     def ts_offload_sync(self):
         _check(lib.ts_offload_sync(self._h), "ts_offload_sync")
+
+    # ---- migration between worker processes (include/turbochunk.h): everything that crosses the process boundary is
+    #      plain Python data (bytes, ints, lists), so it can go through any pipe or socket
+    def ts_pool_export(self):
+        """This pool's registration blob (bytes) for the other worker's ts_peer_open."""
+        blob = ts_pool_export_t()
+        _check(lib.ts_pool_export(self._h, C.byref(blob)), "ts_pool_export")
+        return bytes(blob.bytes)
+
+    def ts_peer_open(self, blob):
+        """Maps the pool another process exported; returns an opaque peer handle (int) for import / release."""
+        b = ts_pool_export_t()
+        C.memmove(b.bytes, bytes(blob), len(b.bytes))
+        peer = C.c_void_p()
+        _check(lib.ts_peer_open(self._h, C.byref(b), C.byref(peer)), "ts_peer_open")
+        self._peers.append(peer.value)
+        return peer.value
+
+    def ts_peer_close(self, peer):
+        self._peers.remove(peer)
+        _check(lib.ts_peer_close(C.c_void_p(peer)), "ts_peer_close")
+
+    def ts_session_freeze(self, sid):
+        """(i) freeze: returns the ticket {"sid", "frames", "head_off", "pages"} to send to the target worker."""
+        cap = max(1, self.ts_session_info(sid)["n_pages"])
+        t = ts_migration_ticket_t()
+        pages = (C.c_int32 * cap)()
+        _check(lib.ts_session_freeze(self._h, sid, C.byref(t), pages, cap), "ts_session_freeze")
+        return {"sid": t.sid, "frames": t.frames, "head_off": t.head_off, "pages": list(pages[:t.n_pages])}
+
+    def ts_session_unfreeze(self, sid):
+        _check(lib.ts_session_unfreeze(self._h, sid), "ts_session_unfreeze")
+
+    def ts_session_import(self, peer, ticket):
+        """(ii) fetch + verify on the target: returns the session's id in this pool."""
+        t = ts_migration_ticket_t(int(ticket["sid"]), int(ticket["frames"]), int(ticket["head_off"]), len(ticket["pages"]))
+        new = C.c_int32(-1)
+        _check(lib.ts_session_import(self._h, C.c_void_p(peer), C.byref(t), _i32(ticket["pages"]), C.byref(new)),
+               "ts_session_import")
+        return new.value
+
+    def ts_session_release(self, sid, peer=None):
+        """(iii) ownership flip on the source, after the target has returned from ts_session_import."""
+        _check(lib.ts_session_release(self._h, sid, C.c_void_p(peer) if peer is not None else C.c_void_p(0)),
+               "ts_session_release")
 
     # ---- introspection
     def ts_session_info(self, sid):

@@ -113,6 +113,8 @@ struct Session {
   uint64_t side_seq = 0;            // last side-stream copy that touched the session
   uint64_t ver = 0;                 // new value whenever P, o or pt change (keys the attention schedule cache)
   bool in_plan = false;             // between ts_step_plan_prepare and ts_step_plan_commit: no other call may touch it
+  bool frozen = false;              // between ts_session_freeze and ts_session_release / _unfreeze (in_plan is set too, so
+                                    // every other call refuses the session)
 };
 
 struct Staging {      // pinned (mapped) host + device buffer pair for per-call schedule records
@@ -196,6 +198,11 @@ struct ts_pool {
   std::vector<tc::WorkItem> sched_items;
   int64_t sched_builds = 0;
   unsigned long long* clock_probe = nullptr;   // ts_pool_clock_probe
+  // migration between worker processes (ts_pool_export): interprocess events, recorded on the side stream
+  cudaEvent_t ipc_frozen = nullptr;            // "state frozen": after the compute work of the last frozen session
+  cudaEvent_t ipc_installed = nullptr;         // "installed": after the last fetch into this pool
+  bool exported = false;
+  ts_pool_export_t export_blob;
 };
 
 namespace tc {
@@ -383,6 +390,8 @@ int ts_pool_destroy(ts_pool* pool) {
     if (e) cudaEventDestroy(e);
   pool->tl_compute.destroy();
   pool->tl_side.destroy();
+  if (pool->ipc_frozen) cudaEventDestroy(pool->ipc_frozen);
+  if (pool->ipc_installed) cudaEventDestroy(pool->ipc_installed);
   if (pool->own_side && pool->side) cudaStreamDestroy(pool->side);
   if (pool->side_out) cudaStreamDestroy(pool->side_out);
   if (pool->own_slab && pool->slab) cudaFree(pool->slab);
@@ -1785,6 +1794,278 @@ int ts_chunk_attention_static(ts_pool* pool, int32_t layer, int32_t n, const int
   const AttnParams p = make_params(pool, L, d, n, 0, layer, k, v, out, lse, scale, false, 0);
   TS_CUDA(launch_attention(p, c.head_dim, grid, stream));
   ++pool->launches;
+  return TS_OK;
+}
+
+}  // extern "C"
+
+// --------------------------------------------------------------------------------------------- migration between processes
+// one worker process per GPU; :263: "registers the corresponding state buffers ... the target worker can
+// then fetch the registered state buffers from the source worker through ... one-sided GPU memory access"; :265: freeze at a
+// chunk boundary, fetch + verify, ownership flips after the transfer.  ts_session_migrate does this between two pools of one
+// process; here the two pools live in two processes (on one GPU, or on two GPUs of a node with peer access):
+//   registration  ts_pool_export  -> blob over the control plane ->  ts_peer_open   (CUDA IPC: the source slab becomes an
+//                                                                     ordinary device pointer for page_pull_kernel)
+//   (i)   freeze  ts_session_freeze  on the source  -> ticket (P, o, page ids) over the control plane
+//   (ii)  fetch   ts_session_import  on the target  -> "enqueued" over the control plane
+//   (iii) flip    ts_session_release on the source
+// Every GPU-side dependency is an interprocess event edge (no host wait in either process): the fetch waits for the source's
+// "state frozen" event, the source's side stream waits for the target's "installed" event before its freed pages can be
+// handed to a writer.  The control-plane messages only have to be delivered in order: a wait is enqueued after the record
+// it is meant for has been enqueued in the other process.
+namespace {
+
+struct ExportBlob {
+  uint32_t magic, version;
+  cudaIpcMemHandle_t mem;             // the allocation that holds the slab
+  cudaIpcEventHandle_t frozen, installed;
+  int64_t slab_offset;                // slab start inside that allocation
+  int64_t page_bytes;
+  int32_t n_layers, n_heads, head_dim, page_tokens, frame_tokens, window_frames, n_pages, pad;
+};
+static_assert(sizeof(ExportBlob) <= sizeof(ts_pool_export_t), "ts_pool_export_t too small");
+constexpr uint32_t kExportMagic = 0x54534950u;   // "TSIP"
+
+typedef CUresult (*PFN_addr_range)(CUdeviceptr*, size_t*, CUdeviceptr);
+PFN_addr_range get_addr_range() {
+  static PFN_addr_range fn = nullptr;
+  if (fn == nullptr) {
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_addr_range>(ptr);
+  }
+  return fn;
+}
+
+int ensure_export(ts_pool* pool) {
+  if (pool->exported) return TS_OK;
+  TS_CUDA(cudaSetDevice(pool->cfg.device));
+  PFN_addr_range range = get_addr_range();
+  CUdeviceptr base = 0;
+  size_t size = 0;
+  if (range == nullptr || range(&base, &size, (CUdeviceptr)pool->slab) != CUDA_SUCCESS) {
+    tc::g_last_cuda_error = "cuMemGetAddressRange(kv slab) failed";
+    return TS_ERR_CUDA;
+  }
+  ExportBlob b;
+  memset(&b, 0, sizeof(b));
+  b.magic = kExportMagic;
+  b.version = 1;
+  TS_CUDA(cudaIpcGetMemHandle(&b.mem, (void*)base));
+  if (pool->ipc_frozen == nullptr)
+    TS_CUDA(cudaEventCreateWithFlags(&pool->ipc_frozen, cudaEventDisableTiming | cudaEventInterprocess));
+  if (pool->ipc_installed == nullptr)
+    TS_CUDA(cudaEventCreateWithFlags(&pool->ipc_installed, cudaEventDisableTiming | cudaEventInterprocess));
+  TS_CUDA(cudaIpcGetEventHandle(&b.frozen, pool->ipc_frozen));
+  TS_CUDA(cudaIpcGetEventHandle(&b.installed, pool->ipc_installed));
+  // an event that was never recorded counts as complete: a waiter that comes first does not block
+  b.slab_offset = (int64_t)((CUdeviceptr)pool->slab - base);
+  b.page_bytes = pool->page_bytes;
+  const ts_pool_config& c = pool->cfg;
+  b.n_layers = c.n_layers;
+  b.n_heads = c.n_heads;
+  b.head_dim = c.head_dim;
+  b.page_tokens = c.page_tokens;
+  b.frame_tokens = c.frame_tokens;
+  b.window_frames = c.window_frames;
+  b.n_pages = c.n_pages;
+  memset(&pool->export_blob, 0, sizeof(pool->export_blob));
+  memcpy(&pool->export_blob, &b, sizeof(b));
+  pool->exported = true;
+  return TS_OK;
+}
+
+}  // namespace
+
+struct ts_peer {
+  ts_pool* local = nullptr;
+  uint8_t* base = nullptr;       // cudaIpcOpenMemHandle mapping of the remote allocation
+  uint8_t* slab = nullptr;       // the remote pool's slab inside it
+  cudaEvent_t frozen = nullptr, installed = nullptr;
+  int32_t n_pages = 0;
+};
+
+extern "C" {
+
+int ts_pool_export(ts_pool* pool, ts_pool_export_t* out) {
+  if (pool == nullptr || out == nullptr) return TS_ERR_INVALID;
+  const int rc = ensure_export(pool);
+  if (rc != TS_OK) return rc;
+  *out = pool->export_blob;
+  return TS_OK;
+}
+
+int ts_peer_open(ts_pool* local, const ts_pool_export_t* remote, ts_peer** out) {
+  if (local == nullptr || remote == nullptr || out == nullptr) return TS_ERR_INVALID;
+  ExportBlob b;
+  memcpy(&b, remote, sizeof(b));
+  const ts_pool_config& c = local->cfg;
+  if (b.magic != kExportMagic || b.version != 1) return TS_ERR_INVALID;
+  if (b.n_layers != c.n_layers || b.n_heads != c.n_heads || b.head_dim != c.head_dim || b.page_tokens != c.page_tokens ||
+      b.frame_tokens != c.frame_tokens || b.window_frames != c.window_frames || b.page_bytes != local->page_bytes ||
+      b.n_pages < 1 || b.slab_offset < 0)
+    return TS_ERR_INVALID;
+  int rc = ensure_export(local);   // the local pool's own events are needed on both ends of a move
+  if (rc != TS_OK) return rc;
+  TS_CUDA(cudaSetDevice(c.device));
+  ts_peer* peer = new ts_peer();
+  peer->local = local;
+  peer->n_pages = b.n_pages;
+  void* base = nullptr;
+  if (!tc::cuda_ok(cudaIpcOpenMemHandle(&base, b.mem, cudaIpcMemLazyEnablePeerAccess), "cudaIpcOpenMemHandle(remote kv slab)") ||
+      !tc::cuda_ok(cudaIpcOpenEventHandle(&peer->frozen, b.frozen), "cudaIpcOpenEventHandle(frozen)") ||
+      !tc::cuda_ok(cudaIpcOpenEventHandle(&peer->installed, b.installed), "cudaIpcOpenEventHandle(installed)")) {
+    if (base) cudaIpcCloseMemHandle(base);
+    if (peer->frozen) cudaEventDestroy(peer->frozen);
+    delete peer;
+    return TS_ERR_CUDA;
+  }
+  peer->base = (uint8_t*)base;
+  peer->slab = peer->base + b.slab_offset;
+  *out = peer;
+  return TS_OK;
+}
+
+int ts_peer_close(ts_peer* peer) {
+  if (peer == nullptr) return TS_ERR_INVALID;
+  cudaSetDevice(peer->local->cfg.device);
+  cudaStreamSynchronize(peer->local->side);     // no fetch of ours still reads the mapping
+  if (peer->frozen) cudaEventDestroy(peer->frozen);
+  if (peer->installed) cudaEventDestroy(peer->installed);
+  if (peer->base) cudaIpcCloseMemHandle(peer->base);
+  cudaGetLastError();
+  delete peer;
+  return TS_OK;
+}
+
+int ts_session_freeze(ts_pool* src, int32_t sid, ts_migration_ticket_t* ticket, int32_t* pages_out, int32_t cap) {
+  if (src == nullptr || ticket == nullptr || (pages_out == nullptr && cap > 0) || cap < 0) return TS_ERR_INVALID;
+  if (sid < 0 || sid >= src->cfg.max_sessions) return TS_ERR_STATE;
+  Session& s = src->sess[sid];
+  if (s.state != TS_SESSION_RESIDENT || s.in_plan) return TS_ERR_STATE;
+  if ((size_t)cap < s.pt.size()) return TS_ERR_INVALID;
+  int rc = ensure_export(src);
+  if (rc != TS_OK) return rc;
+  TS_CUDA(cudaSetDevice(src->cfg.device));
+  // (i) chunk boundary: "state frozen" = after the compute work already enqueued on the session and after a resume of it
+  // that may still be copying in
+  TS_CUDA(src->tl_compute.wait(src->side, s.compute_seq));
+  TS_CUDA(src->tl_side.wait(src->side, s.side_seq));
+  TS_CUDA(cudaEventRecord(src->ipc_frozen, src->side));
+  s.in_plan = s.frozen = true;
+  ticket->sid = sid;
+  ticket->frames = s.P;
+  ticket->head_off = s.o;
+  ticket->n_pages = (int32_t)s.pt.size();
+  std::copy(s.pt.begin(), s.pt.end(), pages_out);
+  return TS_OK;
+}
+
+int ts_session_unfreeze(ts_pool* src, int32_t sid) {
+  if (src == nullptr) return TS_ERR_INVALID;
+  if (sid < 0 || sid >= src->cfg.max_sessions || !src->sess[sid].frozen) return TS_ERR_STATE;
+  src->sess[sid].in_plan = src->sess[sid].frozen = false;
+  return TS_OK;
+}
+
+int ts_session_import(ts_pool* dst, ts_peer* source, const ts_migration_ticket_t* ticket, const int32_t* pages,
+                      int32_t* sid_out) {
+  if (dst == nullptr || source == nullptr || ticket == nullptr || sid_out == nullptr || source->local != dst)
+    return TS_ERR_INVALID;
+  const ts_pool_config& c = dst->cfg;
+  const int64_t n = ticket->n_pages;
+  // (ii) "verifies": the ticket describes a state this geometry can hold, and every page id lies inside the source slab
+  if (n < 0 || (n > 0 && pages == nullptr) || ticket->frames < 0 || ticket->head_off < 0 || ticket->head_off >= c.page_tokens ||
+      n * c.page_tokens < (int64_t)ticket->head_off + (int64_t)ticket->frames * c.frame_tokens ||
+      (c.window_frames > 0 && ticket->frames > c.window_frames))
+    return TS_ERR_INVALID;
+  for (int64_t i = 0; i < n; ++i)
+    if (pages[i] < 0 || pages[i] >= source->n_pages) return TS_ERR_INVALID;
+  int new_sid = -1;
+  for (int i = 0; i < c.max_sessions && new_sid < 0; ++i)
+    if (dst->sess[i].state == TS_SESSION_CLOSED) new_sid = i;
+  if (new_sid < 0) return TS_ERR_CAPACITY;
+  if ((size_t)n > dst->free_q.size()) return TS_ERR_NO_PAGES;
+  TS_CUDA(cudaSetDevice(c.device));
+  Staging* st = nullptr;
+  if (n > 0) {
+    const int rc = acquire_staging(dst, (size_t)n * 8, &st);
+    if (rc != TS_OK) return rc;
+  }
+  Session& t = dst->sess[new_sid];
+  t = Session();
+  t.P = ticket->frames;
+  t.o = ticket->head_off;
+  uint64_t wait_compute = 0, wait_dst_side = 0;
+  for (int64_t i = 0; i < n; ++i) {
+    const int32_t pg = dst->free_q.front();
+    dst->free_q.pop_front();
+    wait_compute = std::max(wait_compute, dst->page_compute_seq[pg]);
+    wait_dst_side = std::max(wait_dst_side, dst->page_side_seq[pg]);
+    t.pt.push_back(pg);
+  }
+  auto undo = [&]() {
+    for (auto it = t.pt.rbegin(); it != t.pt.rend(); ++it) dst->free_q.push_front(*it);
+    t = Session();
+    return TS_ERR_CUDA;
+  };
+#define TS_CUDA_UNDO(call)                    \
+  do {                                        \
+    if (!tc::cuda_ok((call), #call)) return undo(); \
+  } while (0)
+  if (n > 0) {
+    int32_t* pairs = reinterpret_cast<int32_t*>(st->h);
+    for (int64_t i = 0; i < n; ++i) {
+      pairs[2 * i] = pages[i];
+      pairs[2 * i + 1] = t.pt[(size_t)i];
+    }
+    TS_CUDA_UNDO(cudaStreamWaitEvent(dst->side, source->frozen, 0));   // the source's "state frozen"
+    TS_CUDA_UNDO(dst->tl_compute.wait(dst->side, wait_compute));
+    TS_CUDA_UNDO(dst->tl_side.wait(dst->side, wait_dst_side));
+    TS_CUDA_UNDO(launch_upload(st->h_dev, st->d, align_up((size_t)n * 8, 16), dst->side));
+    ++dst->launches;
+    PullParams p;
+    p.src_slab = source->slab;
+    p.dst_slab = dst->slab;
+    p.pairs = reinterpret_cast<const int32_t*>(st->d);
+    p.n_pages = (int32_t)n;
+    p.vec_per_page = (int32_t)(dst->page_bytes / 16);
+    p.page_stride = dst->page_bytes;
+    TS_CUDA_UNDO(launch_page_pull(p, dst->sm_count, dst->side));
+    ++dst->launches;
+    cuda_ok(cudaEventRecord(st->ev, dst->side), "cudaEventRecord");
+    st->in_flight = true;
+    t.side_seq = dst->tl_side.record(dst->side);   // compute calls on the new session wait for the fetch
+  }
+#undef TS_CUDA_UNDO
+  // "installed": what the source's side stream waits for before its pages can be rewritten (also for an empty session, so
+  // that a release always has a record to wait for)
+  cuda_ok(cudaEventRecord(dst->ipc_installed, dst->side), "cudaEventRecord(installed)");
+  t.ver = ++dst->ver_seq;
+  t.state = TS_SESSION_RESIDENT;
+  *sid_out = new_sid;
+  return TS_OK;
+}
+
+int ts_session_release(ts_pool* src, int32_t sid, ts_peer* target) {
+  if (src == nullptr || (target != nullptr && target->local != src)) return TS_ERR_INVALID;
+  if (sid < 0 || sid >= src->cfg.max_sessions || !src->sess[sid].frozen) return TS_ERR_STATE;
+  Session& s = src->sess[sid];
+  TS_CUDA(cudaSetDevice(src->cfg.device));
+  // (iii) ownership flips; the freed pages may be handed to a writer only after the target's fetch has completed
+  uint64_t seq_src = s.side_seq;
+  if (target != nullptr) {
+    TS_CUDA(cudaStreamWaitEvent(src->side, target->installed, 0));
+    seq_src = src->tl_side.record(src->side);
+  }
+  for (int32_t pg : s.pt) {
+    src->page_side_seq[pg] = seq_src;
+    src->page_compute_seq[pg] = s.compute_seq;
+    src->free_q.push_back(pg);
+  }
+  s = Session();
   return TS_OK;
 }
 

@@ -1,0 +1,186 @@
+"""Session migration between two WORKER PROCESSES (PAPER.md:66, :271 one worker per GPU; :263-265 registration, freeze,
+one-sided fetch + verify, ownership flip) against the oracle's `OraclePool.migrate_to`: ids, page tables, free lists and
+logical KV bytes bit-exact on both workers; attention on the target within the north_star tolerance.
+
+Two processes (paper_2606_19271_b200.worker), each with its own CUDA context and pool on the one GPU of the box; the source
+slab reaches the target's fetch kernel through CUDA IPC; "state frozen" and "installed" are interprocess events, so neither
+process waits on the host anywhere in a move.  The parent plays the control plane and holds the oracle pools.  Both worker
+slabs are NaN-poisoned and sit between guard bands."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from helpers import make_oracle_pool, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+MAX_ABS, REL_L2 = 2e-2, 5e-3
+NAN_BF16 = 0x7FC0
+
+
+class Side:
+    """One worker process + the oracle pool that mirrors it."""
+
+    def __init__(self, shape, free_order):
+        from paper_2606_19271_b200 import worker
+        self.shape = shape
+        self.o = make_oracle_pool(shape, free_order)
+        self.w = worker.spawn(device=0)
+        self.w.call("create", n_layers=shape.n_layers, n_heads=shape.n_heads, head_dim=shape.head_dim,
+                    page_tokens=shape.page_tokens, n_pages=shape.n_pages, frame_tokens=shape.frame_tokens,
+                    window_frames=shape.window_frames, max_sessions=shape.max_sessions, free_order=free_order,
+                    guard_bytes=1 << 20, poison=NAN_BF16)
+
+    def open(self):
+        a, b = self.o.open(), self.w.call("pool", "ts_session_open")
+        assert a == b
+        return a
+
+    def append(self, sids, cf, rng, sync=True):
+        """One committed chunk per session of `sids` on every layer (commit on the last)."""
+        from paper_2606_19271_b200 import TS_COMMIT
+        sh = self.shape
+        n = sum(cf) * sh.frame_tokens
+        for layer in range(sh.n_layers):
+            k, v = (synth.draw_bits(rng, n, sh.n_heads, sh.head_dim) for _ in range(2))
+            last = layer == sh.n_layers - 1
+            self.o.append(layer, sids, cf, k, v, commit=last)
+            self.w.call("append", layer, sids, cf, k, v, TS_COMMIT if last else 0)
+
+    def check(self, sids):
+        assert self.w.call("pool", "ts_pool_free_list") == [int(x) for x in self.o.free]
+        for sid in sids:
+            assert self.w.call("pool", "ts_session_page_table", sid) == self.o.page_table(sid)
+            info = self.w.call("pool", "ts_session_info", sid)
+            oi = self.o.info(sid)
+            assert (info["frames"], info["head_off"], info["n_pages"]) == (oi["frames"], oi["head_off"], oi["n_pages"])
+            for layer in range(self.shape.n_layers):
+                gk, gv = self.w.call("gather", layer, sid)
+                ok, ov = self.o.gather_kv(layer, sid)
+                assert np.array_equal(gk.reshape(ok.shape), ok) and np.array_equal(gv.reshape(ov.shape), ov)
+        assert self.w.call("pool", "check_guards"), "a library write strayed outside the KV slab"
+
+    def attention(self, layer, sids, cf, rng, scale):
+        sh = self.shape
+        n = sum(cf) * sh.frame_tokens
+        q, k, v = (synth.draw_bits(rng, n, sh.n_heads, sh.head_dim) for _ in range(3))
+        ref, _ = oracle.chunk_attention(self.o, layer, sids, cf, q, k, v, scale)
+        bits = self.w.call("attention", layer, sids, cf, q, k, v, float(scale))
+        got = synth.bf16_bits_to_f64(bits).reshape(ref.shape)
+        assert np.isfinite(got).all()
+        assert float(np.abs(got - ref).max()) <= MAX_ABS and rel_l2(got, ref) <= REL_L2
+
+    def close(self):
+        self.w.close()
+
+
+def move(src, sid, dst, peer_src_on_dst, peer_dst_on_src):
+    """freeze -> ticket -> import -> "enqueued" -> release, no synchronisation anywhere; the oracle does migrate_to."""
+    ticket = src.w.call("pool", "ts_session_freeze", sid)
+    assert ticket["pages"] == src.o.page_table(sid)
+    new = dst.w.call("pool", "ts_session_import", peer_src_on_dst, ticket)
+    src.w.call("pool", "ts_session_release", sid, peer_dst_on_src)
+    assert new == src.o.migrate_to(sid, dst.o)
+    return new
+
+
+@pytest.fixture
+def pair():
+    sides = []
+
+    def make(shape_a, order_a, shape_b, order_b):
+        sides.append(Side(shape_a, order_a))
+        sides.append(Side(shape_b, order_b))
+        a, b = sides
+        blob_a, blob_b = a.w.call("pool", "ts_pool_export"), b.w.call("pool", "ts_pool_export")
+        assert isinstance(blob_a, bytes) and len(blob_a) == 320
+        return a, b, b.w.call("pool", "ts_peer_open", blob_a), a.w.call("pool", "ts_peer_open", blob_b)
+
+    yield make
+    for s in sides:
+        s.close()
+
+
+def test_session_moves_between_two_worker_processes_and_back(pair):
+    NL, H, D, T, B, W = 2, 3, 128, 100, 64, 7
+    rng = np.random.default_rng(60)
+    sh_a = synth.PoolShape(NL, H, D, B, 72, T, W, 6)
+    sh_b = synth.PoolShape(NL, H, D, B, 56, T, W, 4)      # another pool size: page ids differ on the two sides
+    a, b, a_on_b, b_on_a = pair(sh_a, rng.permutation(72), sh_b, rng.permutation(56))
+    scale = np.float32(1.0 / np.sqrt(D))
+    s0, s1, s2 = a.open(), a.open(), a.open()
+    x0 = b.open()
+    a.append([s0, s1, s2], [2, 3, 1], rng)
+    a.append([s1], [3], rng)                       # s1: 6 frames, window 7
+    b.append([x0], [2], rng)
+    a.check([s0, s1, s2])
+    b.check([x0])
+
+    # the move is requested right behind a committed append on the session: "state frozen" has to cover it
+    a.append([s1], [1], rng)                       # 7 frames: the window is full
+    t1 = move(a, s1, b, a_on_b, b_on_a)
+    b.check([x0, t1])
+    a.check([s0, s2])
+    b.attention(1, [t1, x0], [2, 1], rng, scale)   # the migrated session serves its next chunk on the target
+    # the freed pages of the source are handed out again at once (appends on other sessions), the freed id too
+    a.append([s0, s2], [3, 3], rng)
+    s3 = a.open()
+    assert s3 == s1
+    a.append([s3], [2], rng)
+    a.check([s0, s2, s3])
+    # the session lives on at the target: the window rolls (pages return to the target's free list), then it moves back
+    b.append([t1, x0], [2, 1], rng)
+    b.check([x0, t1])
+    back = move(b, t1, a, b_on_a, a_on_b)
+    a.check([s0, s2, s3, back])
+    b.check([x0])
+    a.attention(0, [back, s0, s3], [1, 2, 3], rng, scale)
+    # a frozen session is held: every other call on it is refused, and the move can be called off
+    from paper_2606_19271_b200 import TS_ERR_STATE
+    from paper_2606_19271_b200.worker import WorkerError
+    ticket = a.w.call("pool", "ts_session_freeze", s0)
+    for call in (("pool", "ts_session_suspend", s0), ("pool", "ts_session_close", s0), ("pool", "ts_session_freeze", s0)):
+        with pytest.raises(WorkerError) as err:
+            a.w.call(*call)
+        assert err.value.code == TS_ERR_STATE
+    a.w.call("pool", "ts_session_unfreeze", s0)
+    a.attention(0, [s0], [1], rng, scale)
+    a.check([s0, s2, s3, back])
+    del ticket
+
+
+def test_import_verifies_the_ticket_and_leaves_the_target_unchanged_on_refusal(pair):
+    from paper_2606_19271_b200 import TS_ERR_INVALID, TS_ERR_NO_PAGES
+    from paper_2606_19271_b200.worker import WorkerError
+    H, D, T, B = 2, 64, 40, 16
+    rng = np.random.default_rng(61)
+    sh_a = synth.PoolShape(1, H, D, B, 40, T, 0, 4)
+    sh_b = synth.PoolShape(1, H, D, B, 12, T, 0, 4)       # too small for the 6-frame session (15 pages)
+    a, b, a_on_b, b_on_a = pair(sh_a, None, sh_b, None)
+    s = a.open()
+    a.append([s], [3], rng)
+    a.append([s], [3], rng)
+    x = b.open()
+    b.append([x], [1], rng)
+    ticket = a.w.call("pool", "ts_session_freeze", s)
+    with pytest.raises(WorkerError) as err:
+        b.w.call("pool", "ts_session_import", a_on_b, ticket)
+    assert err.value.code == TS_ERR_NO_PAGES
+    for bad in (dict(ticket, head_off=B), dict(ticket, frames=ticket["frames"] + 4), dict(ticket, pages=[0, 1, 40]),
+                dict(ticket, pages=[-1] + ticket["pages"][1:])):
+        with pytest.raises(WorkerError) as err:
+            b.w.call("pool", "ts_session_import", a_on_b, bad)
+        assert err.value.code == TS_ERR_INVALID
+    b.check([x])                                          # nothing changed on the target
+    a.w.call("pool", "ts_session_unfreeze", s)            # the move is called off: the session serves on at the source
+    a.append([s], [1], rng)
+    a.check([s])
+    # a geometry mismatch is caught at registration
+    c = Side(synth.PoolShape(1, H, D, 32, 12, T, 0, 4), None)
+    try:
+        with pytest.raises(WorkerError) as err:
+            c.w.call("pool", "ts_peer_open", a.w.call("pool", "ts_pool_export"))
+        assert err.value.code == TS_ERR_INVALID
+    finally:
+        c.close()
