@@ -6,8 +6,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libturbochunk.so")
-SOURCES = ["pool.cu", "kv_copy.cu", "attention_sm100.cu", "attention_qt.cu", "sched.cpp"]
-HEADERS = ["internal.h", "ptx.cuh", "kv_copy.cuh", "attention_common.cuh", os.path.join("..", "..", "include", "turbochunk.h"),
+SOURCES = ["pool.cu", "kv_copy.cu", "attention_sm100.cu", "sched.cpp"]
+HEADERS = ["internal.h", "ptx.cuh", "kv_copy.cuh", os.path.join("..", "..", "include", "turbochunk.h"),
            os.path.join("..", "..", "include", "turbochunk_sched.h")]
 
 

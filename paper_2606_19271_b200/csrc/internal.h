@@ -102,9 +102,6 @@ cudaError_t launch_append(const CopyParams& p, int sm_count, cudaStream_t stream
 cudaError_t launch_gather(const CopyParams& p, int sm_count, cudaStream_t stream);
 cudaError_t launch_page_pull(const PullParams& p, int sm_count, cudaStream_t stream);
 cudaError_t launch_upload(const void* src_mapped, void* dst, size_t bytes, cudaStream_t stream);
-cudaError_t launch_attention_qt(const AttnParams& p, int head_dim, int grid, cudaStream_t stream);
-cudaError_t attention_qt_configure(int head_dim);
-int attention_variant();   // 0: query-tile pairs (attention_sm100.cu), 1: single tiles, Q in TMEM (attention_qt.cu)
 int attention_smem_bytes(int head_dim);
 cudaError_t attention_configure(int head_dim);   // sets the kernel's dynamic shared memory limit on the current device (idempotent)
 

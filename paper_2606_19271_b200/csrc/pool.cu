@@ -736,8 +736,8 @@ static void build_schedule(ts_pool* pool, int32_t n, const int32_t* sids, const 
     }
     return plan;
   };
-  Plan plan = make_plan(attention_variant() == 1 ? 1 : 2);
-  if (attention_variant() == 0 && n * H * 2 <= grid_max) {               // small batch: fewer than two streams per cluster
+  Plan plan = make_plan(2);
+  if (n * H * 2 <= grid_max) {               // small batch: fewer than two streams per cluster
     Plan fine = make_plan(1);
     if (fine.makespan * 108 < plan.makespan * 100) plan = std::move(fine);   // single tiles cost ~8 % more per FLOP
   }
