@@ -63,6 +63,18 @@ def test_invalid_config_rejected_before_cuda(tc):
     assert tc.lib.ts_step_plan_destroy(None) == tc.TS_ERR_INVALID
     assert tc.lib.ts_step_plan_block_bytes(None) == 0
     assert tc.lib.ts_pool_clock_probe(None, None) == tc.TS_ERR_INVALID and tc.lib.ts_pool_sched_builds(None) == 0
+    # the allocation-free attention entry and the cross-process migration calls: null handles are refused before any CUDA call
+    assert tc.lib.ts_static_scratch_bytes() == 256 * 1024
+    assert tc.lib.ts_chunk_attention_static(None, 0, 0, None, None, None, None, None, None, None, C.c_float(1.0), None) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_pool_export(None, None) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_peer_open(None, None, None) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_peer_close(None) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_session_freeze(None, 0, None, None, 0) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_session_unfreeze(None, 0) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_session_import(None, None, None, None, None) == tc.TS_ERR_INVALID
+    assert tc.lib.ts_session_release(None, 0, None) == tc.TS_ERR_INVALID
+    from paper_2606_19271_b200.binding import ts_migration_ticket_t, ts_pool_export_t
+    assert C.sizeof(ts_pool_export_t) == 320 and C.sizeof(ts_migration_ticket_t) == 16      # as include/turbochunk.h declares
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
