@@ -331,7 +331,8 @@ int ts_session_migrate(ts_pool* src, int32_t sid, ts_pool* dst, int32_t* sid_out
  *                   allocation - not from a virtual-memory allocator).  Idempotent.  TS_ERR_CUDA if IPC is unavailable.
  * ts_peer_open    : maps the remote slab into `local`'s process; TS_ERR_INVALID if the blob is malformed or the geometry
  *                   (NL, H, D, B, T, W) differs from `local`'s.  A blob cannot be opened in the process that exported it.
- * ts_peer_close   : waits for `local`'s side stream, then unmaps.
+ * ts_peer_close   : waits for `local`'s side stream, then unmaps.  Every peer opened on a blob must be closed before the pool
+ *                   that exported it is destroyed (CUDA IPC: the exporter keeps the memory alive for its importers).
  * ts_session_freeze : (i).  sid RESIDENT and not held by a step plan (else TS_ERR_STATE).  Records "state frozen" on the
  *                   source's side stream behind the compute work already enqueued on the session; from here until
  *                   release / unfreeze every other call on the session is TS_ERR_STATE.  Writes the ticket and the
