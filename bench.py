@@ -1190,6 +1190,8 @@ def measure_migration_ipc(wl, hbm_peak):
             sids, where = new, where ^ 1
         for w in ws:
             w.call("sync")
+        for w, peer in zip(ws, peers):   # mappings go before the pools that exported them
+            w.call("pool", "ts_peer_close", peer)
     finally:
         for w in ws:
             w.close()

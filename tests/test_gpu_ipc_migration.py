@@ -87,7 +87,7 @@ def move(src, sid, dst, peer_src_on_dst, peer_dst_on_src):
 
 @pytest.fixture
 def pair():
-    sides = []
+    sides, peers = [], []
 
     def make(shape_a, order_a, shape_b, order_b):
         sides.append(Side(shape_a, order_a))
@@ -95,9 +95,12 @@ def pair():
         a, b = sides
         blob_a, blob_b = a.w.call("pool", "ts_pool_export"), b.w.call("pool", "ts_pool_export")
         assert isinstance(blob_a, bytes) and len(blob_a) == 320
-        return a, b, b.w.call("pool", "ts_peer_open", blob_a), a.w.call("pool", "ts_peer_open", blob_b)
+        peers.extend([(b, b.w.call("pool", "ts_peer_open", blob_a)), (a, a.w.call("pool", "ts_peer_open", blob_b))])
+        return a, b, peers[0][1], peers[1][1]
 
     yield make
+    for side, peer in peers:        # every mapping of a slab goes before the pool that exported it
+        side.w.call("pool", "ts_peer_close", peer)
     for s in sides:
         s.close()
 
