@@ -484,6 +484,7 @@ def main():
         result["migrate_p2p"] = measure_migration_p2p(wl)
     if extras:
         result["sustained"] = measure_sustained(wl, out, kclock, device, sust_peak, peak)
+        result["static_entry"] = measure_static_entry(wl, out)
         result["overlap"] = measure_overlap(wl, out)
         pool.close()
         wl["pool"] = None
@@ -692,6 +693,37 @@ def measure_sustained(wl, out, kclock, device, sust_peak, burst_peak, seconds=2.
             "frac_of_nominal_2250": round(tfl / NOMINAL_BF16_TFLOPS, 4), "sm_mhz_in_kernel": mhz,
             "nvml": {"sm_mhz_median": c.get("sm_mhz"), "sm_mhz_min": c.get("sm_min_mhz"), "reasons": c.get("reasons")},
             "peak_kind": "bf16_tflops_sustained (MEASURED_PEAKS.json): cuBLAS back to back for 4 s"}
+
+
+def measure_static_entry(wl, out, reps=20):
+    """ts_chunk_attention_static (no allocation: the schedule block in the library's static device array, copied there from
+    pageable host memory) against ts_chunk_attention on the same batch: ms per call, calls back to back, events on the
+    compute stream.  Outputs are compared bit for bit."""
+    import torch
+    pool = wl["pool"]
+    scale = float(wl["w"].scale)
+    args = (0, wl["sids"], wl["cf"], wl["q"], wl["k"], wl["v"])
+    out2 = torch.empty_like(out)
+    res = {}
+    for name, fn, o in (("ts_chunk_attention", pool.ts_chunk_attention, out),
+                        ("ts_chunk_attention_static", pool.ts_chunk_attention_static, out2)):
+        for _ in range(3):
+            fn(*args, o, None, scale)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        a.record()
+        for _ in range(reps):
+            fn(*args, o, None, scale)
+        b.record()
+        host_ms = (time.perf_counter() - t0) * 1e3 / reps
+        torch.cuda.synchronize()
+        res[name] = {"ms_per_call": round(a.elapsed_time(b) / reps, 4), "host_ms_per_call": round(host_ms, 4)}
+    res["bit_identical"] = bool(torch.equal(out.view(torch.int16), out2.view(torch.int16)))
+    res["static_scratch_bytes"] = 256 * 1024
+    res["note"] = ("host_ms_per_call of the static entry includes waiting for the stream: its block is copied from pageable "
+                   "host memory (no pinned staging to allocate)")
+    return res
 
 
 def measure_overlap(wl, out, reps=12):
