@@ -22,15 +22,15 @@ NAN_BF16 = 0x7FC0
 class Side:
     """One worker process + the oracle pool that mirrors it."""
 
-    def __init__(self, shape, free_order):
+    def __init__(self, shape, free_order, host_pages=32):
         from paper_2606_19271_b200 import worker
         self.shape = shape
-        self.o = make_oracle_pool(shape, free_order)
+        self.o = make_oracle_pool(shape, free_order, host_pages)
         self.w = worker.spawn(device=0)
         self.w.call("create", n_layers=shape.n_layers, n_heads=shape.n_heads, head_dim=shape.head_dim,
                     page_tokens=shape.page_tokens, n_pages=shape.n_pages, frame_tokens=shape.frame_tokens,
                     window_frames=shape.window_frames, max_sessions=shape.max_sessions, free_order=free_order,
-                    guard_bytes=1 << 20, poison=NAN_BF16)
+                    host_pages=host_pages, guard_bytes=1 << 20, poison=NAN_BF16)
 
     def open(self):
         a, b = self.o.open(), self.w.call("pool", "ts_session_open")
@@ -187,3 +187,47 @@ def test_import_verifies_the_ticket_and_leaves_the_target_unchanged_on_refusal(p
         assert err.value.code == TS_ERR_INVALID
     finally:
         c.close()
+
+
+def test_many_moves_with_chunks_in_between(pair):
+    """Three sessions wander between the two workers for 30 moves while they keep generating chunks (windows roll, page
+    tables wrap around both free lists, freed ids and pages are reused at once); state and bytes against the oracle every
+    tenth move and at the end, attention on both workers at the end."""
+    from paper_2606_19271_b200 import TS_ERR_STATE
+    from paper_2606_19271_b200.worker import WorkerError
+    NL, H, D, T, B, W = 1, 2, 64, 50, 16, 5
+    rng = np.random.default_rng(62)
+    sh = synth.PoolShape(NL, H, D, B, 80, T, W, 4)
+    a, b, a_on_b, b_on_a = pair(sh, rng.permutation(80), sh, rng.permutation(80))
+    sides = [a, b]
+    peer_of_src_on = {0: b_on_a, 1: a_on_b}     # peer handle held by side i for the OTHER side's pool
+    where = {}                                  # session tag -> (side index, sid)
+    for tag in range(3):
+        sid = a.open()
+        a.append([sid], [int(rng.integers(1, 4))], rng)
+        where[tag] = (0, sid)
+    scale = np.float32(1.0 / np.sqrt(D))
+    for mv in range(30):
+        tag = int(rng.integers(0, 3))
+        i, sid = where[tag]
+        src, dst = sides[i], sides[1 - i]
+        if rng.random() < 0.6:
+            src.append([sid], [int(rng.integers(1, 3))], rng)          # the move follows a chunk without any wait
+        if rng.random() < 0.2:                                         # a suspended session does not move (PAPER.md:265)
+            src.w.call("pool", "ts_session_suspend", sid)
+            src.o.suspend(sid)
+            with pytest.raises(WorkerError) as err:
+                src.w.call("pool", "ts_session_freeze", sid)
+            assert err.value.code == TS_ERR_STATE
+            src.w.call("pool", "ts_session_resume", sid)
+            src.o.resume(sid)
+        new = move(src, sid, dst, peer_of_src_on[1 - i], peer_of_src_on[i])
+        where[tag] = (1 - i, new)
+        if mv % 10 == 9:
+            for k, side in enumerate(sides):
+                side.check(sorted(s for (w, s) in where.values() if w == k))
+    for k, side in enumerate(sides):
+        mine = sorted(s for (w, s) in where.values() if w == k)
+        side.check(mine)
+        if mine:
+            side.attention(0, mine, [1] * len(mine), rng, scale)
