@@ -64,6 +64,13 @@ def serve(conn, device):
                 pool.ts_chunk_attention(layer, sids, cf, dq, _to_dev(k, dev), _to_dev(v, dev), out, None, float(scale))
                 torch.cuda.synchronize(dev)
                 res = _to_bits(out)
+            elif op == "chunk_step":      # (layer, sids, cf, q_bits, k_bits, v_bits, scale, flags) -> out bits (one fused launch)
+                layer, sids, cf, q, k, v, scale, flags = args
+                dq = _to_dev(q, dev)
+                out = torch.full_like(dq, float("nan"))
+                pool.ts_chunk_step(layer, sids, cf, dq, _to_dev(k, dev), _to_dev(v, dev), out, None, float(scale), flags)
+                torch.cuda.synchronize(dev)
+                res = _to_bits(out)
             elif op == "gather":          # (layer, sid) -> (k bits, v bits) in logical order
                 gk, gv = pool.ts_gather_kv(*args)
                 torch.cuda.synchronize(dev)

@@ -231,3 +231,88 @@ def test_many_moves_with_chunks_in_between(pair):
         side.check(mine)
         if mine:
             side.attention(0, mine, [1] * len(mine), rng, scale)
+
+
+def test_scheduler_drives_three_worker_processes():
+    """TurboServe in miniature, deployed as the paper deploys it: a session manager (this
+    process: the ownership table, the closed-loop scheduler of Algorithm 1) and three GPU worker PROCESSES.  Every decision
+    epoch the scheduler places the sessions and sets the budget; the manager carries the decisions out over the pipes -
+    open / close, suspend of idle sessions, resume, freeze -> import -> release for every net migration - and every worker
+    then runs one coalesced chunk step (one fused launch) for its active sessions.  The oracle (SchedulerOracle + one
+    OraclePool per worker) is driven by the same events: decisions, page tables, free lists and KV bytes identical,
+    attention within the north_star tolerance."""
+    import paper_2606_19271_b200 as tc
+    from test_scheduler_parity import event_stream, same
+    T, K, M_max = 96, 3, 3
+    shape = synth.PoolShape(n_layers=1, n_heads=2, head_dim=128, page_tokens=64, n_pages=K * 12 + 8, frame_tokens=T,
+                            window_frames=6, max_sessions=K + 2)
+    rng = np.random.default_rng(12)
+    workers = [Side(shape, rng.permutation(shape.n_pages), host_pages=40 * 9) for _ in range(M_max)]
+    peers = {}
+    try:
+        blobs = [w.w.call("pool", "ts_pool_export") for w in workers]
+        for i in range(M_max):                    # peers[(i, j)]: worker j's pool as seen from worker i
+            for j in range(M_max):
+                if i != j:
+                    peers[(i, j)] = workers[i].w.call("pool", "ts_peer_open", blobs[j])
+        cfg = dict(K=K, M_max=M_max, M0=1, l_hat=[0, 90, 174, 267], rho_hat=0.7, delta=0.1, eta=0.01, kappa_alpha=5.0,
+                   kappa_beta=0.05)
+        so, sg = oracle.SchedulerOracle(**cfg), tc.TurboSched(**cfg)
+        scale = np.float32(1.0 / np.sqrt(128.0))
+        where, suspended = {}, set()              # the ownership table: session uid -> (worker, local sid)
+        n_mig = n_steps = n_resume = 0
+        for it, ev in enumerate(event_stream(seed=5, n_events=60, cap=K * M_max, mean_on=2.0, mean_off=0.5, p_leave=0.06)):
+            a, b = so.event(ev), sg.ts_sched_event(ev)
+            same(a, b)
+            live = {uid for uid, _, _ in ev}
+            for uid in [u for u in where if u not in live]:                     # terminated
+                w, sid = where.pop(uid)
+                workers[w].o.close(sid)
+                workers[w].w.call("pool", "ts_session_close", sid)
+                suspended.discard(uid)
+            for uid, alpha, _ in ev:
+                g = b["phi"][uid]
+                if uid not in where:
+                    if g >= 0:
+                        where[uid] = (g, workers[g].open())
+                    continue
+                w, sid = where[uid]
+                if g < 0:
+                    if uid not in suspended and not alpha:                      # went idle: offload, release the slot
+                        workers[w].o.suspend(sid)
+                        workers[w].w.call("pool", "ts_session_suspend", sid)
+                        suspended.add(uid)
+                    continue
+                if uid in suspended:                                            # reactivated: restore where the copy is ...
+                    workers[w].o.resume(sid)
+                    workers[w].w.call("pool", "ts_session_resume", sid)
+                    suspended.discard(uid)
+                    n_resume += 1
+                if g != w:                                                      # ... and move to the worker PLACE chose
+                    where[uid] = (g, move(workers[w], sid, workers[g], peers[(g, w)], peers[(w, g)]))
+                    n_mig += 1
+            for g in b["alive"]:                                                # one coalesced chunk step per worker
+                batch = sorted(sid for uid, (w, sid) in where.items() if w == g and b["phi"].get(uid, -1) == g)
+                if not batch:
+                    continue
+                cf = [int(rng.integers(1, 3)) for _ in batch]
+                q, k, v = (synth.draw_bits(rng, sum(cf) * T, shape.n_heads, shape.head_dim) for _ in range(3))
+                side = workers[g]
+                ref, _ = oracle.chunk_attention(side.o, 0, batch, cf, q, k, v, scale)
+                side.o.append(0, batch, cf, k, v)
+                got = synth.bf16_bits_to_f64(side.w.call("chunk_step", 0, batch, cf, q, k, v, float(scale), tc.TS_COMMIT))
+                got = got.reshape(ref.shape)
+                assert float(np.abs(got - ref).max()) <= MAX_ABS and rel_l2(got, ref) <= REL_L2
+                n_steps += 1
+            if it % 6 == 5 or it == 59:
+                for g, side in enumerate(workers):
+                    side.check([sid for uid, (w, sid) in where.items() if w == g and uid not in suspended])
+        assert n_mig >= 3 and n_resume >= 2 and n_steps >= 40, (n_mig, n_resume, n_steps)
+    finally:
+        for (i, j), peer in peers.items():
+            try:
+                workers[i].w.call("pool", "ts_peer_close", peer)
+            except Exception:
+                pass
+        for w in workers:
+            w.close()
