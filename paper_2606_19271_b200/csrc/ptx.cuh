@@ -75,6 +75,24 @@ __device__ __forceinline__ void mbar_wait_long(uint64_t* bar, uint32_t parity) {
         : "memory");
   } while (!ok);
 }
+// Non-blocking test in a tight loop: the waiter reacts to the completion at once instead of being woken (~140 clk with
+// try_wait), but keeps issuing meanwhile.  Only for a wait that is short AND on the critical path: the MMA thread's wait for the
+// second half of P (-1.2 % SM cycles per launch; on its other waits, or in the softmax warps, the issue slots it takes from the
+// scheduler's other warps cost more than the wake-up saves: profiles/r2_step_timeline.md).
+__device__ __forceinline__ void mbar_spin(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) {
   }
