@@ -343,7 +343,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
             if (j < 2) mbar_wait(&o_free[i], ((i ? cnt_it1 : cnt_it0) & 1) ^ 1);
             tc_fence_after();
             issue_pv_half(i, slot_v, 0, j >= 2);
-            mbar_spin(&p_half[2 * i + 1], par);   // short and on the critical path: spin
+            mbar_poll(&p_half[2 * i + 1], par);   // short and on the critical path: poll
             tc_fence_after();
             issue_pv_half(i, slot_v, 1, true);
             mma_commit(&o_done[i]);
@@ -395,7 +395,7 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
             if (j == 0) mbar_wait(&o_free[i], ((i ? cnt_it1 : cnt_it0) & 1) ^ 1);
             tc_fence_after();
             issue_pv_half(i, slot_v, 0, j > 0);
-            mbar_spin(&p_half[2 * i + 1], par);   // short and on the critical path: spin
+            mbar_poll(&p_half[2 * i + 1], par);   // short and on the critical path: poll
             tc_fence_after();
             issue_pv_half(i, slot_v, 1, true);
             mma_commit(&o_done[i]);

@@ -75,13 +75,14 @@ __device__ __forceinline__ void mbar_wait_long(uint64_t* bar, uint32_t parity) {
         : "memory");
   } while (!ok);
 }
-// Non-blocking test in a tight loop: the waiter reacts to the completion at once instead of being woken (~140 clk with
-// try_wait), but keeps issuing meanwhile.  Only for a wait that is short AND on the critical path: the MMA thread's wait for the
-// second half of P (-1.2 % SM cycles per launch; on its other waits, or in the softmax warps, the issue slots it takes from the
-// scheduler's other warps cost more than the wake-up saves: profiles/r2_step_timeline.md).
-__device__ __forceinline__ void mbar_spin(uint64_t* bar, uint32_t parity) {
+// Polling wait: a non-blocking test, then a nap of ~16 ns, until the phase has completed.  The waiter reacts within a few
+// dozen clocks instead of being woken (~140 clk with try_wait) and, unlike a tight test loop, leaves nearly all issue slots to
+// the other warps of its scheduler.  Only for a wait that is short AND on the critical path: the MMA thread's wait for the
+// second half of P (-2.2 % SM cycles per launch; a tight loop gives -1.2 %, naps of 32 / 64 ns -1.5 % / -0.3 %; the same wait
+// on the thread's other barriers or in the softmax warps loses: profiles/r2_step_timeline.md, r2_cycle_experiments.md).
+__device__ __forceinline__ void mbar_poll(uint64_t* bar, uint32_t parity) {
   uint32_t ok;
-  do {
+  for (;;) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
@@ -91,7 +92,9 @@ __device__ __forceinline__ void mbar_spin(uint64_t* bar, uint32_t parity) {
         : "=r"(ok)
         : "r"(smem_u32(bar)), "r"(parity)
         : "memory");
-  } while (!ok);
+    if (ok) break;
+    asm volatile("nanosleep.u32 %0;" ::"r"(16u));
+  }
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) {
