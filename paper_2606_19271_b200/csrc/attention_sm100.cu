@@ -282,28 +282,30 @@ __global__ void __launch_bounds__(kThreads, 1) chunk_attention_kernel(const __gr
     if (elect_one()) {
       constexpr uint32_t idesc_s = make_idesc_bf16(128, 128, 0, 0);
       constexpr uint32_t idesc_pv = make_idesc_bf16(128, D, 0, 1);
-      const uint32_t sQ_addr = smem_u32(sQ);
-      const uint32_t sKV_addr = smem_u32(sKV);
+      // operand addresses in 16-byte units, reduced ONCE to the descriptor's 14-bit field (a shared-memory address carries the
+      // CTA's rank within the cluster above bit 18): from here on descriptor arithmetic is plain addition
+      const uint32_t sQ16 = (smem_u32(sQ) >> 4) & 0x3FFFu;
+      const uint32_t sKV16 = (smem_u32(sKV) >> 4) & 0x3FFFu;
       // S of TMEM tile slot `i` = (query tile `qi` in smem) x (K tile in ring slot `slot`)^T
       auto issue_s_q = [&](int qi, int i, uint32_t slot) {
-        const uint32_t a = sQ_addr + qi * C::kTileBytes;
-        const uint32_t b = sKV_addr + slot * C::kTileBytes;
+        const uint32_t a = sQ16 + qi * (C::kTileBytes >> 4);
+        const uint32_t b = sKV16 + slot * (C::kTileBytes >> 4);
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk) {
-          const uint32_t off = (kk >> 2) * C::kBlockBytes + (kk & 3) * 32;
-          mma_ss(tmem_base + i * 128, make_smem_desc_sw128(a + off, 16, 1024), make_smem_desc_sw128(b + off, 16, 1024),
+          const uint32_t off = (kk >> 2) * (C::kBlockBytes >> 4) + (kk & 3) * 2;
+          mma_ss(tmem_base + i * 128, make_smem_desc_sw128_a16(a + off, 16, 1024), make_smem_desc_sw128_a16(b + off, 16, 1024),
                  idesc_s, kk > 0);
         }
       };
       auto issue_s = [&](int i, uint32_t slot) { issue_s_q(i, i, slot); };
       // half h of O_i += P_i V: the 16-key steps 4h .. 4h+3 (keys [64h, 64h+64))
       auto issue_pv_half = [&](int i, uint32_t slot, int h, bool acc) {
-        const uint32_t b = sKV_addr + slot * C::kTileBytes;
+        const uint32_t b = sKV16 + slot * (C::kTileBytes >> 4);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           const int kk = 4 * h + q;
           mma_ts(tmem_base + 256 + i * D, tmem_base + i * 128 + kk * 8,
-                 make_smem_desc_sw128(b + kk * 2048, C::kBlockBytes, 1024), idesc_pv, (acc || q > 0) ? 1u : 0u);
+                 make_smem_desc_sw128_a16(b + kk * 128, C::kBlockBytes, 1024), idesc_pv, (acc || q > 0) ? 1u : 0u);
         }
       };
       uint32_t kv_it = 0, q_cnt = 0;

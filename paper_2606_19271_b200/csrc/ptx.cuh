@@ -190,6 +190,15 @@ __device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t saddr, uint32_
   d |= (uint64_t)2 << 61;
   return d;
 }
+// The same descriptor from the address in 16-byte units, built by ADDITION instead of shift / mask / or: shared-memory
+// addresses are below 256 KB, so the 14-bit address field cannot carry into the next one, and "base + offset" of a tile walk
+// folds into one add per instruction on the issuing thread (it was four uniform-datapath operations per descriptor, in front
+// of every batch of MMAs: on the critical path right after the wait for P).
+__device__ __forceinline__ uint64_t make_smem_desc_sw128_a16(uint32_t saddr16, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  const uint32_t lo = saddr16 + ((lbo_bytes >> 4) << 16);
+  const uint32_t hi = (sbo_bytes >> 4) | (1u << 14) | (2u << 29);
+  return ((uint64_t)hi << 32) | lo;
+}
 // Instruction descriptor, kind::f16: D = fp32, A = B = bf16.  a_mn / b_mn: 0 = K-major, 1 = MN-major.
 __host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N, int a_mn, int b_mn) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)b_mn << 16) |
