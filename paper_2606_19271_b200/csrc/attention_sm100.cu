@@ -97,7 +97,9 @@ __device__ __forceinline__ int next_cluster_item(const AttnParams& p, uint32_t k
     int idx = atomicAdd(p.feed_hdr, 1);
     if (idx >= __ldg(p.feed_hdr + 2)) idx = -1;
     const unsigned long long v = ((unsigned long long)(k + 1) << 32) | (uint32_t)(idx + 1);
-    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(slot), "l"(v) : "memory");
+    // relaxed: the 64-bit word IS the message (sequence number and item index); the records it points to were written by the
+    // host before the launch.  An acquire on the reading side would invalidate L1 at every poll for nothing.
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(slot), "l"(v) : "memory");
     if (idx < 0 && atomicAdd(p.feed_hdr + 1, 1) == (int)(gridDim.x >> 1) - 1) {
       p.feed_hdr[1] = 0;
       p.feed_hdr[0] = 0;
@@ -106,7 +108,7 @@ __device__ __forceinline__ int next_cluster_item(const AttnParams& p, uint32_t k
   }
   unsigned long long v;
   do {
-    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(slot) : "memory");
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(slot) : "memory");
   } while ((uint32_t)(v >> 32) != k + 1);
   return (int)(uint32_t)v - 1;
 }
