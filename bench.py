@@ -43,7 +43,7 @@ FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustain
 COMMIT_EVERY = 4
 # dram__bytes_read.sum + dram__bytes_write.sum of one attention launch on this workload, from the ncu --set full
 # capture summarised in the file named beside it (not a measurement of this run).
-ATTENTION_DRAM_TRAFFIC = {"bytes": 1544758000, "from": "profiles/r2_attention.txt (ncu --set full, the fused launch: 1.2065 GB read + 338.2 MB "
+ATTENTION_DRAM_TRAFFIC = {"bytes": 1543272000, "from": "profiles/r2_attention.txt (ncu --set full, final build, the fused launch: 1.2028 GB read + 340.5 MB "
                                                           "written; attention-only launch 1.038 GB, profiles/r1_final_build.txt)"}
 
 
