@@ -457,6 +457,9 @@ def main():
                      "frac_of_nominal_2250": round(achieved / NOMINAL_BF16_TFLOPS, 4),
                      "ms_per_launch": round(attn_ms, 4), "timed_in": "the loop `value` comes from (events around each launch)",
                      "sm_mhz_in_kernel": clock_in_kernel,
+                     # FLOP per SM clock against the tensor pipe's 8192 per SM: does not depend on the clock the box grants
+                     "tensor_frac_of_cycles": (round(achieved * 1e12 / (148 * 8192 * clock_in_kernel * 1e6), 4)
+                                               if clock_in_kernel else None),
                      "traffic": ATTENTION_DRAM_TRAFFIC["bytes"], "traffic_from": ATTENTION_DRAM_TRAFFIC["from"]},
         "kernels_alone": {"note": "separate launches, second loop after a 0.5 s idle gap (another power state)",
                           "attention_ms": round(attn_alone_ms, 4),
