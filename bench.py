@@ -482,7 +482,10 @@ def main():
                                       if k in ("d2h", "h2d", "placement")}
     result["migrate"] = measure_migration(wl, peaks["hbm_gbs"])
     if extras:
-        result["migrate_ipc"] = measure_migration_ipc(wl, peaks["hbm_gbs"])
+        try:      # two extra processes and CUDA IPC: a box that refuses either must not cost the run its headline line
+            result["migrate_ipc"] = measure_migration_ipc(wl, peaks["hbm_gbs"])
+        except Exception as exc:
+            result["migrate_ipc"] = {"unavailable": f"{type(exc).__name__}: {exc}"[:300]}
     if world > 1 and torch.cuda.device_count() >= 2:
         result["migrate_p2p"] = measure_migration_p2p(wl)
     if extras:
