@@ -117,7 +117,7 @@ class Worker:
         """Send without waiting for the reply (collect it with result()): lets two workers run side by side."""
         self.conn.send((op, args, kw))
 
-    def result(self, timeout=600):
+    def result(self, timeout=180):
         if not self.conn.poll(timeout):
             raise WorkerError("worker did not answer", None)
         rep = self.conn.recv()
